@@ -1,0 +1,164 @@
+/* u1gf.h -- C-ABI boundary of libu1gf.so: B200-native (sm_100a) lattice-Landau-gauge relaxation and
+ * Gribov-copy counting for compact U(1), the hot path of Mehta & Schroeck, "Enumerating Copies in the
+ * First Gribov Region on the Lattice in up to four Dimensions" (arXiv:1403.0555).
+ *
+ * Citations are PAPER.md:L<line> (+ section / equation); R<k> are the readings listed in DESIGN.md section 3.
+ *
+ * Conventions common to every call
+ *   - plain C, no exceptions cross the boundary.  Return value 0 = success, negative = error code below;
+ *     u1gf_last_error() then returns a thread-local, NUL-terminated description valid until the next call.
+ *   - "dev" pointers are CUDA device pointers owned by the CALLER (e.g. torch tensors); "host" pointers are
+ *     ordinary host memory owned by the caller.  Only the orbit handle is library-owned.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-pointer calls
+ *     are asynchronous on that stream and never synchronise the device; `*_host` calls copy results back and
+ *     return after the stream has drained.
+ *   - there is NO CPU fallback: without a usable sm_100 device every compute call returns U1GF_ENODEV.
+ *   - site index i = x0 + N0*(x1 + N1*(x2 + N2*x3)), periodic in every direction;
+ *     link angle theta_{i,mu} at [i*d + mu]; complex numbers are interleaved (re, im) doubles.
+ *   - gauge-transformed link U^g_{i,mu} = g_i U_{i,mu} conj(g_{i+mu}) (Eq. 5 convention, R1); the functional
+ *     F[g] = sum_{i,mu} Re U^g_{i,mu} is MAXIMISED (Eq. 3, x_paper = 1 - F/(dV)).
+ *   - per start, results are a pure function of (orbit, seed, start index, omega, eps, max_sweeps, check_every):
+ *     no floating-point atomics, fixed reduction trees; independent of launch configuration and of which other
+ *     starts run beside it.
+ */
+#ifndef U1GF_H
+#define U1GF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define U1GF_OK 0
+#define U1GF_EINVAL (-1) /* bad argument (message says which) */
+#define U1GF_ENODEV (-2) /* no CUDA device of compute capability 10.x */
+#define U1GF_ECUDA (-3)  /* a CUDA runtime call failed (message carries cudaGetErrorString) */
+#define U1GF_ENOMEM (-4) /* host or device allocation failed / workspace too small */
+
+typedef struct u1gf_orbit u1gf_orbit; /* opaque, library-owned */
+
+const char* u1gf_last_error(void);
+
+/* Version of this ABI (bumped on incompatible change). */
+int u1gf_abi_version(void);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * a1  Orbit setup.  One gauge orbit = one link field on a periodic lattice.
+ *   d           number of dimensions, 1..4 (the paper uses 2..4; d = 1 is accepted for the ring closed form)
+ *   extents     host [d], each >= 2, V = prod extents <= 8192
+ *   theta_host  host [V*d] link angles in radians, any range (only cos/sin are used)
+ *   out         receives the handle.  U = (cos theta, sin theta) is evaluated on the host with libm and copied
+ *               to the current CUDA device together with neighbour / update-phase tables.  Synchronous.
+ * Update order (R3): sites are grouped into phases (parity, level) such that a phase contains no two
+ * neighbouring sites; for all-even extents these are the two checkerboard colours of PAPER.md:L99.
+ * ------------------------------------------------------------------------------------------------------- */
+int u1gf_create_orbit(int d, const int32_t* extents, const double* theta_host, u1gf_orbit** out);
+int u1gf_destroy_orbit(u1gf_orbit* o);
+/* Volume V and dimension d of a handle (0 on NULL). */
+int32_t u1gf_orbit_volume(const u1gf_orbit* o);
+int32_t u1gf_orbit_dim(const u1gf_orbit* o);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * a2-a6  Relaxation of a batch of random starts (Eq. 4-5; R2, R5, R6).
+ * Start with index s: g_i = exp(i*pi*(2u-1)), u the 53-bit uniform of Philox4x32-10 with key (seed lo, seed hi)
+ * and counter (i, s lo, s hi, 0) (PAPER.md:L121 names Philox).  Sweep: for each phase in order, every site of
+ * the phase gets w_i = sum_mu [conj(U_{i,mu}) g_{i+mu} + U_{i-mu,mu} g_{i-mu}] (= conj K_i, Eq. 5),
+ * g_i <- normalise((1-omega) g_i + omega w_i/|w_i|) (over-relaxation R2; omega = 1 is the paper's
+ * algorithm); a site with |w_i|^2 < 1e-280 is left unchanged (R6).  After sweep t with t % check_every == 0 the
+ * gauge precision vartheta = (1/V) sum_i Delta_i^2, Delta_i = Im(g_i conj w_i), is tested against eps (R5).
+ *   seed, first_start, n_starts   start k uses index start_ids[k] if start_ids != NULL else first_start + k
+ *   start_ids   dev [n_starts] or NULL
+ *   omega       in [1, 2);  eps > 0;  max_sweeps >= 1;  check_every >= 1
+ *   F_norm      dev [n]    F/(dV) of the final field
+ *   sweeps      dev [n]    number of full sweeps performed
+ *   status      dev [n]    bit0: max_sweeps reached without passing the test; bit1: an R6 skip occurred
+ *   sig         dev [n*4]  canonical signature: g~_i = g_i conj(g_{V-1}) (angle at the last site (N,..,N) fixed to
+ *                          zero); p_k = (1/V) sum_i (a_{k,i} Re g~_i + b_{k,i} Im g~_i), k = 0..3,
+ *                          a, b in {+1,-1} from Philox key (0x51, 0) counter (i, k, 0, 1), bit 0 of words 0 / 1
+ *   g_canon     dev [n*V*2] canonical fields g~, or NULL (16 GiB at 2^22 starts of 4^4: normally NULL, and only
+ *               the representatives are re-relaxed with start_ids to obtain their fields)
+ *   workspace   dev scratch of at least u1gf_relax_workspace_bytes(o, n_starts) bytes, 256-byte aligned; its
+ *               contents are undefined afterwards.  Nothing is allocated inside the call.
+ * Errors: EINVAL on NULL / out-of-range arguments, ENOMEM if workspace_bytes is too small, ECUDA on launch failure.
+ * ------------------------------------------------------------------------------------------------------- */
+size_t u1gf_relax_workspace_bytes(const u1gf_orbit* o, uint64_t n_starts);
+int u1gf_relax_batch(const u1gf_orbit* o, uint64_t seed, uint64_t first_start, uint64_t n_starts,
+                     const uint64_t* start_ids, double omega, double eps, int32_t max_sweeps, int32_t check_every,
+                     double* F_norm, int32_t* sweeps, uint8_t* status, double* sig, double* g_canon,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream);
+/* Same computation with HOST result arrays (and host start_ids or NULL): device buffers and workspace are
+ * allocated inside, results copied back, stream drained before returning.  Any output pointer may be NULL. */
+int u1gf_relax_batch_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_start, uint64_t n_starts,
+                          const uint64_t* start_ids_host, double omega, double eps, int32_t max_sweeps,
+                          int32_t check_every, double* F_norm_host, int32_t* sweeps_host, uint8_t* status_host,
+                          double* sig_host, double* g_canon_host);
+
+/* Kernel selection for u1gf_relax_batch on this handle: 0 = automatic (specialised resident kernel when one
+ * exists for the extents, else the generic one), 1 = force the generic kernel.  Results per start are the same
+ * copies either way; the two kernels may differ in the last bits of F and, rarely, by a sweep (R14). */
+int u1gf_set_kernel(u1gf_orbit* o, int32_t which);
+/* Name of the kernel u1gf_relax_batch will use for this handle (static string). */
+const char* u1gf_kernel_name(const u1gf_orbit* o);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * a7  First-Gribov-region test (R9).  For each configuration g (unit complex per site):
+ * c_{i,mu} = Re(g_i U_{i,mu} conj g_{i+mu}); Faddeev-Popov operator = Hessian of -F,
+ * (M v)_i = sum_mu [c_{i,mu}(v_i - v_{i+mu}) + c_{i-mu,mu}(v_i - v_{i-mu})]; lambda_1 = smallest eigenvalue of M on
+ * the orthogonal complement of the constant vector (the global gauge zero mode), computed by a
+ * batched matrix-free Lanczos iteration (one CTA per configuration).
+ *   g           dev [n_cfg*V*2]
+ *   tol_fp      region = 1 if lambda_1 > tol_fp (inside), 2 if |lambda_1| <= tol_fp (marginal, "semi"definite),
+ *               0 if lambda_1 < -tol_fp (outside)
+ *   lambda1     dev [n_cfg];  region dev [n_cfg];  n_in_region dev [1] = number of configurations with region != 0
+ * ------------------------------------------------------------------------------------------------------- */
+int u1gf_check_fp(const u1gf_orbit* o, uint64_t n_cfg, const double* g, double tol_fp, double* lambda1,
+                  uint8_t* region, int64_t* n_in_region, void* cuda_stream);
+int u1gf_check_fp_host(const u1gf_orbit* o, uint64_t n_cfg, const double* g_host, double tol_fp,
+                       double* lambda1_host, uint8_t* region_host, int64_t* n_in_region_host);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * a8  De-duplication and counting (PAPER.md:L129-135 sort the functional values and count distinct ones; L149
+ * counts as a function of the number of samples; L167 histogram; R7, R8, R15).  Records with status bit0 set get
+ * copy_id = -1.  The others are sorted by F/(dV) (ties by position), cut into maximal runs with adjacent gaps
+ * <= tol_F; inside a run the unassigned record with the smallest position becomes a leader and takes every
+ * unassigned record whose signature agrees within tol_sig (max norm), repeated until the run is used up.
+ * Copies are numbered in order of first discovery (increasing leader position).
+ *   F_norm dev [n], sig dev [n*4], status dev [n]
+ *   copy_id      dev [n] int32
+ *   n_distinct   dev [1] int64
+ *   rep          dev [n] int64: rep[c] = position of the leader of copy c, c < n_distinct (rest undefined)
+ *   multiplicity dev [n] int64: members of copy c
+ *   hist         dev [nbins] int64 or NULL: histogram over nbins equal bins on [0,1] of F_norm[rep[c]] weighted by
+ *                multiplicity[c] (PAPER.md:L167 uses width 1e-4)
+ *   workspace    dev scratch >= u1gf_count_workspace_bytes(n), 256-byte aligned
+ * ------------------------------------------------------------------------------------------------------- */
+size_t u1gf_count_workspace_bytes(uint64_t n);
+int u1gf_count_copies(uint64_t n, const double* F_norm, const double* sig, const uint8_t* status, double tol_F,
+                      double tol_sig, int32_t* copy_id, int64_t* n_distinct, int64_t* rep, int64_t* multiplicity,
+                      int64_t* hist, int32_t nbins, void* workspace, size_t workspace_bytes, void* cuda_stream);
+int u1gf_count_copies_host(uint64_t n, const double* F_norm_host, const double* sig_host,
+                           const uint8_t* status_host, double tol_F, double tol_sig, int32_t* copy_id_host,
+                           int64_t* n_distinct_host, int64_t* rep_host, int64_t* multiplicity_host,
+                           int64_t* hist_host, int32_t nbins);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Measurement helpers (not part of the method): roofline denominators measured on the device in use.
+ *   u1gf_measure_fp64_peak   runs a dependent-chain-free DFMA kernel on all SMs for about `ms` milliseconds and
+ *                            returns FP64 FMA instructions (thread-level) per second in *dfma_per_s.
+ *   u1gf_measure_smem_peak   same for 128-bit conflict-free shared-memory loads, bytes per second.
+ *   u1gf_last_launch_count   kernels launched by the calling thread's most recent compute call.
+ *   u1gf_last_relax_ms       device time (CUDA events on the call's stream) of the relaxation kernel of the
+ *                            calling thread's most recent u1gf_relax_batch*, after synchronising those events;
+ *                            returns < 0 if none.
+ * ------------------------------------------------------------------------------------------------------- */
+int u1gf_measure_fp64_peak(double ms, double* dfma_per_s, void* cuda_stream);
+int u1gf_measure_smem_peak(double ms, double* bytes_per_s, void* cuda_stream);
+int32_t u1gf_last_launch_count(void);
+double u1gf_last_relax_ms(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* U1GF_H */

@@ -1,0 +1,252 @@
+"""Thin ctypes binding of libu1gf.so (include/u1gf.h): same names, argument marshalling only.
+
+torch supplies device memory and the CUDA stream; every step of the path runs in the library's kernels.
+There is no CPU fallback: if the shared library is missing or no sm_100 device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libu1gf.so")
+
+# every symbol include/u1gf.h declares: name -> (restype, argtypes)
+_p = C.c_void_p
+_SIGNATURES = {
+    "u1gf_last_error": (C.c_char_p, []),
+    "u1gf_abi_version": (C.c_int, []),
+    "u1gf_create_orbit": (C.c_int, [C.c_int, _p, _p, C.POINTER(_p)]),
+    "u1gf_destroy_orbit": (C.c_int, [_p]),
+    "u1gf_orbit_volume": (C.c_int32, [_p]),
+    "u1gf_orbit_dim": (C.c_int32, [_p]),
+    "u1gf_relax_workspace_bytes": (C.c_size_t, [_p, C.c_uint64]),
+    "u1gf_relax_batch": (C.c_int, [_p, C.c_uint64, C.c_uint64, C.c_uint64, _p, C.c_double, C.c_double, C.c_int32,
+                                   C.c_int32, _p, _p, _p, _p, _p, _p, C.c_size_t, _p]),
+    "u1gf_relax_batch_host": (C.c_int, [_p, C.c_uint64, C.c_uint64, C.c_uint64, _p, C.c_double, C.c_double,
+                                        C.c_int32, C.c_int32, _p, _p, _p, _p, _p]),
+    "u1gf_set_kernel": (C.c_int, [_p, C.c_int32]),
+    "u1gf_kernel_name": (C.c_char_p, [_p]),
+    "u1gf_check_fp": (C.c_int, [_p, C.c_uint64, _p, C.c_double, _p, _p, _p, _p]),
+    "u1gf_check_fp_host": (C.c_int, [_p, C.c_uint64, _p, C.c_double, _p, _p, _p]),
+    "u1gf_count_workspace_bytes": (C.c_size_t, [C.c_uint64]),
+    "u1gf_count_copies": (C.c_int, [C.c_uint64, _p, _p, _p, C.c_double, C.c_double, _p, _p, _p, _p, _p, C.c_int32,
+                                    _p, C.c_size_t, _p]),
+    "u1gf_count_copies_host": (C.c_int, [C.c_uint64, _p, _p, _p, C.c_double, C.c_double, _p, _p, _p, _p, _p,
+                                         C.c_int32]),
+    "u1gf_measure_fp64_peak": (C.c_int, [C.c_double, C.POINTER(C.c_double), _p]),
+    "u1gf_measure_smem_peak": (C.c_int, [C.c_double, C.POINTER(C.c_double), _p]),
+    "u1gf_last_launch_count": (C.c_int32, []),
+    "u1gf_last_relax_ms": (C.c_double, []),
+}
+
+_lib = None
+
+
+class U1gfError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libu1gf error {code}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Load libu1gf.so (fails loudly if it was not built: there is no fallback path)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(f"{LIB_PATH} not built; run `python -m paper_1403_0555_b200.build`")
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def exported_symbols():
+    return sorted(_SIGNATURES)
+
+
+def _check(rc):
+    if rc != 0:
+        raise U1gfError(rc, lib().u1gf_last_error().decode())
+
+
+def _np_ptr(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _dev_ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+class Orbit:
+    """u1gf_create_orbit / u1gf_destroy_orbit (a1)."""
+
+    def __init__(self, extents, theta):
+        e = np.ascontiguousarray(extents, dtype=np.int32)
+        t = np.ascontiguousarray(theta, dtype=np.float64).reshape(-1)
+        if t.size != int(np.prod(e)) * e.size:
+            raise ValueError("theta must have V*d entries (index i*d+mu)")
+        h = C.c_void_p()
+        _check(lib().u1gf_create_orbit(int(e.size), _np_ptr(e), _np_ptr(t), C.byref(h)))
+        self.handle = h
+        self.extents = tuple(int(x) for x in e)
+        self.d = int(e.size)
+        self.V = int(np.prod(e))
+
+    def close(self):
+        if getattr(self, "handle", None):
+            lib().u1gf_destroy_orbit(self.handle)
+            self.handle = None
+
+    __del__ = close
+
+    def set_kernel(self, which: int):
+        _check(lib().u1gf_set_kernel(self.handle, int(which)))
+
+    @property
+    def kernel_name(self) -> str:
+        return lib().u1gf_kernel_name(self.handle).decode()
+
+
+def _workspace(nbytes):
+    import torch
+    return torch.empty(max(int(nbytes), 256) + 256, dtype=torch.uint8, device="cuda")
+
+
+def _aligned_ptr(ws):
+    p = ws.data_ptr()
+    return C.c_void_p((p + 255) & ~255)
+
+
+def relax_batch(orbit: Orbit, seed, n_starts, *, first_start=0, start_ids=None, omega=1.7, eps=1e-13,
+                max_sweeps=20000, check_every=1, want_g=False, out=None, workspace=None):
+    """u1gf_relax_batch with device (torch) result tensors.  Returns a dict of torch tensors on the GPU.
+    `out` / `workspace` may carry preallocated tensors from a previous call (nothing is then allocated)."""
+    import torch
+    if start_ids is not None:
+        if not isinstance(start_ids, torch.Tensor):
+            start_ids = torch.as_tensor(np.ascontiguousarray(start_ids, dtype=np.uint64).view(np.int64), device="cuda")
+        n_starts = start_ids.numel()
+    n = int(n_starts)
+    if out is None:
+        out = dict(F_norm=torch.empty(n, dtype=torch.float64, device="cuda"),
+                   sweeps=torch.empty(n, dtype=torch.int32, device="cuda"),
+                   status=torch.empty(n, dtype=torch.uint8, device="cuda"),
+                   sig=torch.empty((n, 4), dtype=torch.float64, device="cuda"),
+                   g_canon=torch.empty((n, orbit.V, 2), dtype=torch.float64, device="cuda") if want_g else None)
+    need = lib().u1gf_relax_workspace_bytes(orbit.handle, n)
+    if workspace is None or workspace.numel() < need + 256:
+        workspace = _workspace(need)
+    out["workspace"] = workspace
+    _check(lib().u1gf_relax_batch(orbit.handle, int(seed), int(first_start), n, _dev_ptr(start_ids), float(omega),
+                                  float(eps), int(max_sweeps), int(check_every), _dev_ptr(out["F_norm"]),
+                                  _dev_ptr(out["sweeps"]), _dev_ptr(out["status"]), _dev_ptr(out["sig"]),
+                                  _dev_ptr(out.get("g_canon")), _aligned_ptr(workspace), need, _stream()))
+    return out
+
+
+def relax_batch_host(orbit: Orbit, seed, n_starts, *, first_start=0, start_ids=None, omega=1.7, eps=1e-13,
+                     max_sweeps=20000, check_every=1, want_g=False):
+    """u1gf_relax_batch_host: numpy result arrays, device<->host copies inside the call."""
+    ids = None
+    if start_ids is not None:
+        ids = np.ascontiguousarray(start_ids, dtype=np.uint64)
+        n_starts = ids.size
+    n = int(n_starts)
+    out = dict(F_norm=np.zeros(n), sweeps=np.zeros(n, dtype=np.int32), status=np.zeros(n, dtype=np.uint8),
+               sig=np.zeros((n, 4)), g_canon=np.zeros((n, orbit.V, 2)) if want_g else None)
+    _check(lib().u1gf_relax_batch_host(orbit.handle, int(seed), int(first_start), n, _np_ptr(ids), float(omega),
+                                       float(eps), int(max_sweeps), int(check_every), _np_ptr(out["F_norm"]),
+                                       _np_ptr(out["sweeps"]), _np_ptr(out["status"]), _np_ptr(out["sig"]),
+                                       _np_ptr(out["g_canon"])))
+    return out
+
+
+def check_fp(orbit: Orbit, g, tol_fp=1e-8):
+    """u1gf_check_fp on a device tensor g[n_cfg, V, 2] -> dict(lambda1, region, n_in_region) of device tensors."""
+    import torch
+    g = g.contiguous()
+    n = int(g.shape[0]) if g.numel() else 0
+    lam = torch.empty(n, dtype=torch.float64, device="cuda")
+    reg = torch.empty(n, dtype=torch.uint8, device="cuda")
+    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    _check(lib().u1gf_check_fp(orbit.handle, n, _dev_ptr(g), float(tol_fp), _dev_ptr(lam), _dev_ptr(reg),
+                               _dev_ptr(cnt), _stream()))
+    return dict(lambda1=lam, region=reg, n_in_region=cnt)
+
+
+def check_fp_host(orbit: Orbit, g, tol_fp=1e-8):
+    g = np.ascontiguousarray(g, dtype=np.float64).reshape(-1, orbit.V, 2)
+    n = g.shape[0]
+    lam = np.zeros(n)
+    reg = np.zeros(n, dtype=np.uint8)
+    cnt = np.zeros(1, dtype=np.int64)
+    _check(lib().u1gf_check_fp_host(orbit.handle, n, _np_ptr(g), float(tol_fp), _np_ptr(lam), _np_ptr(reg),
+                                    _np_ptr(cnt)))
+    return dict(lambda1=lam, region=reg, n_in_region=int(cnt[0]))
+
+
+def count_copies(F_norm, sig, status, tol_F=1e-10, tol_sig=1e-4, nbins=0, workspace=None):
+    """u1gf_count_copies on device tensors -> dict of device tensors (copy_id, n_distinct, rep, multiplicity, hist).
+    rep / multiplicity are full-length; entries beyond n_distinct are undefined."""
+    import torch
+    n = int(F_norm.numel())
+    copy_id = torch.empty(n, dtype=torch.int32, device="cuda")
+    nd = torch.zeros(1, dtype=torch.int64, device="cuda")
+    rep = torch.empty(max(n, 1), dtype=torch.int64, device="cuda")
+    mult = torch.empty(max(n, 1), dtype=torch.int64, device="cuda")
+    hist = torch.empty(nbins, dtype=torch.int64, device="cuda") if nbins else None
+    need = lib().u1gf_count_workspace_bytes(n)
+    if workspace is None or workspace.numel() < need + 256:
+        workspace = _workspace(need)
+    _check(lib().u1gf_count_copies(n, _dev_ptr(F_norm), _dev_ptr(sig), _dev_ptr(status), float(tol_F), float(tol_sig),
+                                   _dev_ptr(copy_id), _dev_ptr(nd), _dev_ptr(rep), _dev_ptr(mult), _dev_ptr(hist),
+                                   int(nbins), _aligned_ptr(workspace), need, _stream()))
+    return dict(copy_id=copy_id, n_distinct=nd, rep=rep, multiplicity=mult, hist=hist, workspace=workspace)
+
+
+def count_copies_host(F_norm, sig, status, tol_F=1e-10, tol_sig=1e-4, nbins=0):
+    F = np.ascontiguousarray(F_norm, dtype=np.float64)
+    S = np.ascontiguousarray(sig, dtype=np.float64).reshape(-1, 4)
+    st = np.ascontiguousarray(status, dtype=np.uint8)
+    n = F.size
+    copy_id = np.zeros(n, dtype=np.int32)
+    nd = np.zeros(1, dtype=np.int64)
+    rep = np.zeros(max(n, 1), dtype=np.int64)
+    mult = np.zeros(max(n, 1), dtype=np.int64)
+    hist = np.zeros(nbins, dtype=np.int64) if nbins else None
+    _check(lib().u1gf_count_copies_host(n, _np_ptr(F), _np_ptr(S), _np_ptr(st), float(tol_F), float(tol_sig),
+                                        _np_ptr(copy_id), _np_ptr(nd), _np_ptr(rep), _np_ptr(mult), _np_ptr(hist),
+                                        int(nbins)))
+    k = int(nd[0])
+    return dict(copy_id=copy_id, n_distinct=k, rep=rep[:k], multiplicity=mult[:k], hist=hist)
+
+
+def measure_fp64_peak(ms=200.0) -> float:
+    v = C.c_double(0)
+    _check(lib().u1gf_measure_fp64_peak(float(ms), C.byref(v), _stream()))
+    return v.value
+
+
+def measure_smem_peak(ms=200.0) -> float:
+    v = C.c_double(0)
+    _check(lib().u1gf_measure_smem_peak(float(ms), C.byref(v), _stream()))
+    return v.value
+
+
+def last_launch_count() -> int:
+    return int(lib().u1gf_last_launch_count())
+
+
+def last_relax_ms() -> float:
+    return float(lib().u1gf_last_relax_ms())

@@ -1,0 +1,279 @@
+// check_fp.cu -- a7 first-Gribov-region test: lowest non-trivial eigenvalue of the Faddeev-Popov operator.
+// PAPER.md:L38 defines M_FP as the Hessian of the gauge-fixing functional, L9/L50 the first Gribov region as the
+// set where it is positive (semi)definite; the constant vector is its exact zero mode (global gauge freedom,
+// PAPER.md:L65).  The paper never evaluates M_FP; north_star asks for lambda_1 per copy by batched Lanczos.
+//
+// One CTA per configuration.  Shared memory holds the link weights c_{i,mu} = Re(g_i U_{i,mu} conj g_{i+mu}) and
+// two Lanczos vectors; the three-term recurrence runs on the orthogonal complement of the constant vector
+// (re-projected every step).  The smallest Ritz value comes from Sturm-count multisection by warp 0, the stop
+// test from the residual bound beta_k |s_k| (last component of the Ritz vector).
+#include "u1gf_internal.h"
+
+namespace u1gf {
+namespace {
+
+constexpr int kMaxK = 512;  // Lanczos steps kept
+
+struct FpParams {
+    unsigned long long n_cfg;
+    const double2* g;
+    double tol_fp;
+    double* lambda1;
+    uint8_t* region;
+    unsigned long long* n_in;
+};
+
+__device__ __forceinline__ double block_sum(double a, double (*red)[32], int& buf) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) a += __shfl_down_sync(0xffffffffu, a, o);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0) red[buf][warp] = a;
+    __syncthreads();
+    double s = 0.0;
+    for (int w = 0; w < nw; ++w) s += red[buf][w];
+    buf ^= 1;
+    return s;
+}
+
+__device__ __forceinline__ void block_sum2(double& a, double& b, double (*red)[32], double (*red2)[32], int& buf) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, o);
+        b += __shfl_down_sync(0xffffffffu, b, o);
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0) {
+        red[buf][warp] = a;
+        red2[buf][warp] = b;
+    }
+    __syncthreads();
+    double sa = 0.0, sb = 0.0;
+    for (int w = 0; w < nw; ++w) {
+        sa += red[buf][w];
+        sb += red2[buf][w];
+    }
+    a = sa;
+    b = sb;
+    buf ^= 1;
+}
+
+// number of eigenvalues of the k x k tridiagonal (alpha[0..k), beta[0..k-1)) below x (Sturm sequence)
+__device__ __forceinline__ int sturm_count(const double* alpha, const double* beta, int k, double x) {
+    int cnt = 0;
+    double q = alpha[0] - x;
+    if (q < 0.0) ++cnt;
+    for (int j = 1; j < k; ++j) {
+        if (fabs(q) < 1e-300) q = 1e-300;
+        q = alpha[j] - x - beta[j - 1] * beta[j - 1] / q;
+        if (q < 0.0) ++cnt;
+    }
+    return cnt;
+}
+
+// Smallest eigenvalue of T_k by 33-way multisection on warp 0 (all 32 lanes call this), bracket [lo, hi].
+__device__ double smallest_ritz(const double* alpha, const double* beta, int k, double lo, double hi) {
+    const int lane = threadIdx.x & 31;
+    for (int it = 0; it < 14; ++it) {
+        const double h = (hi - lo) / 33.0;
+        const double x = lo + h * (double)(lane + 1);
+        const int c = sturm_count(alpha, beta, k, x);
+        const unsigned m = __ballot_sync(0xffffffffu, c >= 1);
+        if (m == 0) {
+            lo = lo + h * 32.0;
+        } else {
+            const int f = __ffs(m) - 1;  // first lane whose x lies above the smallest eigenvalue
+            hi = lo + h * (double)(f + 1);
+            lo = lo + h * (double)f;
+        }
+        if (hi - lo <= 4e-16 * fmax(1.0, fmax(fabs(lo), fabs(hi)))) break;
+    }
+    return 0.5 * (lo + hi);
+}
+
+// |last component| of the normalised eigenvector of T_k for (an approximation from below of) its smallest
+// eigenvalue: s_{j+1} = -(q_j/beta_j) s_j with the Sturm quotients q_j.
+__device__ double last_component(const double* alpha, const double* beta, int k, double lam) {
+    double q = alpha[0] - lam, s = 1.0, norm2 = 1.0;
+    for (int j = 1; j < k; ++j) {
+        if (fabs(q) < 1e-300) q = 1e-300;
+        const double r = -q / beta[j - 1];
+        s *= r;
+        norm2 = fma(s, s, norm2);
+        if (norm2 > 1e200) {  // rescale
+            s *= 1e-100;
+            norm2 *= 1e-200;
+        }
+        q = alpha[j] - lam - beta[j - 1] * beta[j - 1] / q;
+    }
+    return fabs(s) * rsqrt(norm2);
+}
+
+template <int DIM>
+__global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const FpParams P) {
+    extern __shared__ double sm[];
+    const int V = D.V, tid = threadIdx.x, T = blockDim.x;
+    double* c = sm;                 // [V*DIM]
+    double* va = c + (size_t)V * DIM;  // [V]
+    double* vb = va + V;            // [V]
+    __shared__ double red[2][32], red2[2][32];
+    __shared__ double alpha[kMaxK], beta[kMaxK];
+    __shared__ double s_lam, s_res;
+    int buf = 0;
+    const int kmax = min(V - 1, kMaxK);
+
+    for (unsigned long long cfg = blockIdx.x; cfg < P.n_cfg; cfg += gridDim.x) {
+        const double2* g = P.g + cfg * (unsigned long long)V;
+        __syncthreads();
+        for (int l = tid; l < V * DIM; l += T) {
+            const int i = l / DIM, mu = l - i * DIM;
+            const double2 gi = g[i], gj = g[__ldg(D.fwd + l)], u = __ldg(D.U + l);
+            const double ar = gi.x * u.x - gi.y * u.y, ai = gi.x * u.y + gi.y * u.x;
+            c[l] = ar * gj.x + ai * gj.y;
+            (void)mu;
+        }
+        // start vector: fixed pseudo-random signs/values, constant mode removed, normalised
+        double s1 = 0.0;
+        for (int i = tid; i < V; i += T) {
+            const u32x4 r = philox((uint32_t)i, 0u, 0u, 5u, 0x52u, 0u);
+            const double x = unit_interval_pm1(r.x, r.y);
+            va[i] = x;
+            s1 += x;
+        }
+        s1 = block_sum(s1, red, buf);
+        const double mean0 = s1 / (double)V;
+        double s2 = 0.0;
+        for (int i = tid; i < V; i += T) {
+            const double x = va[i] - mean0;
+            va[i] = x;
+            s2 = fma(x, x, s2);
+            vb[i] = 0.0;
+        }
+        s2 = block_sum(s2, red, buf);
+        const double inv0 = rsqrt(s2);
+        for (int i = tid; i < V; i += T) va[i] *= inv0;
+        __syncthreads();
+
+        double* v1 = va;  // current Lanczos vector
+        double* v0 = vb;  // previous one; overwritten by the new direction
+        double beta_prev = 0.0, lam = 0.0, lam_hi = 4.0 * DIM + 1.0;
+        int k = 0, next_check = 8;
+        bool done = false;
+        while (!done) {
+            // w = M v1 - beta_prev v0  (into v0), alpha = <w, v1>
+            double a = 0.0;
+            for (int i = tid; i < V; i += T) {
+                const double vi = v1[i];
+                double acc = 0.0;
+#pragma unroll
+                for (int mu = 0; mu < DIM; ++mu) {
+                    const int jf = __ldg(D.fwd + i * DIM + mu), jb = __ldg(D.bwd + i * DIM + mu);
+                    acc = fma(c[i * DIM + mu], vi - v1[jf], acc);
+                    acc = fma(c[jb * DIM + mu], vi - v1[jb], acc);
+                }
+                const double w = fma(-beta_prev, v0[i], acc);
+                v0[i] = w;
+                a = fma(w, vi, a);
+            }
+            a = block_sum(a, red, buf);
+            // w -= alpha v1 ; remove the constant mode ; beta = |w|
+            double sw = 0.0, sww = 0.0;
+            for (int i = tid; i < V; i += T) {
+                const double w = fma(-a, v1[i], v0[i]);
+                v0[i] = w;
+                sw += w;
+            }
+            sw = block_sum(sw, red, buf);
+            const double mean = sw / (double)V;
+            for (int i = tid; i < V; i += T) {
+                const double w = v0[i] - mean;
+                v0[i] = w;
+                sww = fma(w, w, sww);
+            }
+            sww = block_sum(sww, red, buf);
+            const double b = sqrt(sww);
+            if (tid == 0) {
+                alpha[k] = a;
+                beta[k] = b;
+            }
+            ++k;
+            const bool breakdown = b < 1e-13 * (4.0 * DIM);
+            if (breakdown || k == kmax || k == next_check) {
+                __syncthreads();
+                if (tid < 32) {
+                    const double l = smallest_ritz(alpha, beta, k, -(4.0 * DIM + 1.0), lam_hi);
+                    const double res = breakdown ? 0.0 : b * last_component(alpha, beta, k, l - 1e-13);
+                    if (tid == 0) {
+                        s_lam = l;
+                        s_res = res;
+                    }
+                }
+                __syncthreads();
+                lam = s_lam;
+                lam_hi = lam + 1e-9;  // Ritz values decrease with k (interlacing)
+                if (breakdown || k == kmax || s_res < 1e-10) done = true;
+                next_check = k + max(4, k / 4);
+            }
+            if (!done) {
+                const double ib = 1.0 / b;
+                for (int i = tid; i < V; i += T) v0[i] *= ib;
+                double* tmp = v0;
+                v0 = v1;
+                v1 = tmp;
+                beta_prev = b;
+                __syncthreads();
+            }
+        }
+        if (tid == 0) {
+            P.lambda1[cfg] = lam;
+            const uint8_t reg = lam > P.tol_fp ? 1 : (fabs(lam) <= P.tol_fp ? 2 : 0);
+            P.region[cfg] = reg;
+            if (reg) atomicAdd(P.n_in, 1ull);
+        }
+    }
+}
+
+template <int DIM>
+int launch(const u1gf_orbit* o, const FpParams& P, cudaStream_t st) {
+    const int V = o->dev.V;
+    const size_t smem = ((size_t)V * DIM + 2 * (size_t)V) * sizeof(double);
+    if (smem > 220 * 1024)
+        return fail(U1GF_EINVAL, "u1gf_check_fp: lattice of %d sites does not fit the resident Lanczos kernel", V);
+    auto kern = lanczos_kernel<DIM>;
+    if (smem > 48 * 1024) U1GF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int T = (V + 31) / 32 * 32;
+    if (T > 512) T = 512;
+    int per_sm = 0;
+    U1GF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T, smem));
+    if (per_sm < 1) return fail(U1GF_ECUDA, "u1gf_check_fp: kernel does not fit on an SM");
+    unsigned long long grid = (unsigned long long)per_sm * o->sm_count;
+    if (grid > P.n_cfg) grid = P.n_cfg;
+    kern<<<(unsigned)grid, T, smem, st>>>(o->dev, P);
+    U1GF_CUDA(cudaGetLastError());
+    ++t_launches;
+    return U1GF_OK;
+}
+
+}  // namespace
+}  // namespace u1gf
+
+using namespace u1gf;
+
+extern "C" int u1gf_check_fp(const u1gf_orbit* o, uint64_t n_cfg, const double* g, double tol_fp, double* lambda1,
+                             uint8_t* region, int64_t* n_in_region, void* cuda_stream) {
+    t_launches = 0;
+    if (!o) return fail(U1GF_EINVAL, "u1gf_check_fp: NULL orbit");
+    if (!n_in_region) return fail(U1GF_EINVAL, "u1gf_check_fp: NULL n_in_region");
+    if (!(tol_fp >= 0.0)) return fail(U1GF_EINVAL, "u1gf_check_fp: tol_fp must be >= 0");
+    if (int rc = check_device()) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    U1GF_CUDA(cudaMemsetAsync(n_in_region, 0, sizeof(int64_t), st));
+    if (n_cfg == 0) return U1GF_OK;
+    if (!g || !lambda1 || !region) return fail(U1GF_EINVAL, "u1gf_check_fp: NULL array");
+    FpParams P{n_cfg, (const double2*)g, tol_fp, lambda1, region, (unsigned long long*)n_in_region};
+    switch (o->dev.d) {
+        case 1: return launch<1>(o, P, st);
+        case 2: return launch<2>(o, P, st);
+        case 3: return launch<3>(o, P, st);
+        default: return launch<4>(o, P, st);
+    }
+}
