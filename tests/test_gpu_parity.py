@@ -250,7 +250,7 @@ def test_check_fp_closed_forms_and_regions(b, oracle):
         orbit = b.Orbit(ext, th)
         f = b.check_fp(orbit, torch.as_tensor(g[None], device="cuda"))
         c = np.array([np.cos(2 * np.pi * km / N) for km in k])
-        spec = [sum(2 * c[mu] * (1 - np.cos(2 * np.pi * m[mu] / N)) * (2 if N == 2 else 1) for mu in range(d))
+        spec = [sum(2 * c[mu] * (1 - np.cos(2 * np.pi * m[mu] / N)) for mu in range(d))
                 for m in np.ndindex(*ext) if any(m)]
         lam = float(f["lambda1"][0])
         assert abs(lam - min(spec)) < TOL_LAM, (ext, k, lam, min(spec))
