@@ -1,0 +1,58 @@
+"""Host-side logic of the N > 1 launch.
+
+The path shards over starts: a start's trajectory is a pure function of (orbit, seed, start index, omega,
+eps), and the paper itself runs its GPUs from a host loop over independent samples.  Every rank
+therefore takes a disjoint, contiguous range of start indices of the same orbit and runs the whole hot path on
+it; there is NO data-path collective ("replicas only").  What is exchanged is only the measurement: the step
+time (max over ranks) and the work counters (sum over ranks).
+
+This module holds no arithmetic of the method and works on any torch.distributed backend (nccl on the GPUs,
+gloo in the CPU tests).
+"""
+from __future__ import annotations
+
+import os
+from dataclasses import dataclass
+
+
+@dataclass(frozen=True)
+class RankInfo:
+    rank: int
+    world: int
+    local_rank: int
+
+
+def rank_info_from_env(env=None) -> RankInfo:
+    """RANK / WORLD_SIZE / LOCAL_RANK as torchrun exports them (1 process = 1 GPU); single process if unset."""
+    env = os.environ if env is None else env
+    return RankInfo(int(env.get("RANK", "0")), int(env.get("WORLD_SIZE", "1")), int(env.get("LOCAL_RANK", "0")))
+
+
+def weak_start_range(rank: int, world: int, n_per_rank: int) -> tuple[int, int]:
+    """Weak scaling (bench.py): every rank relaxes `n_per_rank` starts; rank r owns [r*n, (r+1)*n)."""
+    if not (0 <= rank < world) or n_per_rank < 0:
+        raise ValueError("bad rank / world / n_per_rank")
+    return rank * n_per_rank, n_per_rank
+
+
+def strong_start_range(rank: int, world: int, n_total: int) -> tuple[int, int]:
+    """Strong scaling: `n_total` starts split into contiguous ranges whose sizes differ by at most one."""
+    if not (0 <= rank < world) or n_total < 0:
+        raise ValueError("bad rank / world / n_total")
+    q, r = divmod(n_total, world)
+    first = rank * q + min(rank, r)
+    return first, q + (1 if rank < r else 0)
+
+
+def aggregate(total_ms: float, counters, dist=None, device="cpu"):
+    """(max over ranks of total_ms, sum over ranks of each counter).  `dist` is torch.distributed (initialised) or
+    None for a single process.  Counters are summed in float64 (exact below 2^53)."""
+    counters = [float(c) for c in counters]
+    if dist is None:
+        return float(total_ms), counters
+    import torch
+    t = torch.tensor([float(total_ms)], dtype=torch.float64, device=device)
+    c = torch.tensor(counters, dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t[0]), [float(x) for x in c]
