@@ -147,6 +147,11 @@ int u1gf_count_copies_host(uint64_t n, const double* F_norm_host, const double* 
  * Measurement helpers (not part of the method): roofline denominators measured on the device in use.
  *   u1gf_measure_fp64_peak   runs a dependent-chain-free DFMA kernel on all SMs for about `ms` milliseconds and
  *                            returns FP64 FMA instructions (thread-level) per second in *dfma_per_s.
+ *   u1gf_measure_fp64_rate   the same rate for a DFMA stream of a given operand pattern: 0 = the stream of
+ *                            u1gf_measure_fp64_peak (one register operand, two constants); 1 = three distinct
+ *                            register operands per DFMA; 2 = the complex multiply-accumulate pattern of the
+ *                            neighbour sum w_i (Eq. 5).  Patterns 1 and 2 are limited by register-file
+ *                            operand bandwidth, not by the FP64 lanes.
  *   u1gf_measure_smem_peak   same for 128-bit conflict-free shared-memory loads, bytes per second.
  *   u1gf_last_launch_count   kernels launched by the calling thread's most recent compute call.
  *   u1gf_last_relax_ms       device time (CUDA events on the call's stream) of the relaxation kernel of the
@@ -154,6 +159,7 @@ int u1gf_count_copies_host(uint64_t n, const double* F_norm_host, const double* 
  *                            returns < 0 if none.
  * ------------------------------------------------------------------------------------------------------- */
 int u1gf_measure_fp64_peak(double ms, double* dfma_per_s, void* cuda_stream);
+int u1gf_measure_fp64_rate(int32_t pattern, double ms, double* dfma_per_s, void* cuda_stream);
 int u1gf_measure_smem_peak(double ms, double* bytes_per_s, void* cuda_stream);
 int32_t u1gf_last_launch_count(void);
 double u1gf_last_relax_ms(void);

@@ -37,6 +37,7 @@ _SIGNATURES = {
     "u1gf_count_copies_host": (C.c_int, [C.c_uint64, _p, _p, _p, C.c_double, C.c_double, _p, _p, _p, _p, _p,
                                          C.c_int32]),
     "u1gf_measure_fp64_peak": (C.c_int, [C.c_double, C.POINTER(C.c_double), _p]),
+    "u1gf_measure_fp64_rate": (C.c_int, [C.c_int32, C.c_double, C.POINTER(C.c_double), _p]),
     "u1gf_measure_smem_peak": (C.c_int, [C.c_double, C.POINTER(C.c_double), _p]),
     "u1gf_last_launch_count": (C.c_int32, []),
     "u1gf_last_relax_ms": (C.c_double, []),
@@ -108,7 +109,11 @@ class Orbit:
             lib().u1gf_destroy_orbit(self.handle)
             self.handle = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:   # interpreter shutdown: module globals may already be gone
+            pass
 
     def set_kernel(self, which: int):
         _check(lib().u1gf_set_kernel(self.handle, int(which)))
@@ -235,6 +240,12 @@ def count_copies_host(F_norm, sig, status, tol_F=1e-10, tol_sig=1e-4, nbins=0):
 def measure_fp64_peak(ms=200.0) -> float:
     v = C.c_double(0)
     _check(lib().u1gf_measure_fp64_peak(float(ms), C.byref(v), _stream()))
+    return v.value
+
+
+def measure_fp64_rate(pattern: int, ms=200.0) -> float:
+    v = C.c_double(0)
+    _check(lib().u1gf_measure_fp64_rate(int(pattern), float(ms), C.byref(v), _stream()))
     return v.value
 
 
