@@ -96,8 +96,10 @@ int u1gf_relax_batch_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_sta
                           double* sig_host, double* g_canon_host);
 
 /* Kernel selection for u1gf_relax_batch on this handle: 0 = automatic (specialised resident kernel when one
- * exists for the extents, else the generic one), 1 = force the generic kernel.  Results per start are the same
- * copies either way; the two kernels may differ in the last bits of F and, rarely, by a sweep (R14). */
+ * exists for the extents; the streamed lane-per-start kernel for all-even lattices of 512 sites and more; else
+ * the generic one), 1 = force the generic kernel, 2 = force the streamed kernel (all extents even, else generic).
+ * Results per start are the same copies either way; kernels may differ in the last bits of F and, rarely, by a
+ * sweep (R14). */
 int u1gf_set_kernel(u1gf_orbit* o, int32_t which);
 /* Name of the kernel u1gf_relax_batch will use for this handle (static string). */
 const char* u1gf_kernel_name(const u1gf_orbit* o);

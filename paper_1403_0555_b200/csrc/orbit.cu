@@ -206,21 +206,27 @@ int u1gf_destroy_orbit(u1gf_orbit* o) {
 }
 
 int u1gf_set_kernel(u1gf_orbit* o, int32_t which) {
-    if (!o || which < 0 || which > 1) return fail(U1GF_EINVAL, "u1gf_set_kernel: bad argument");
+    if (!o || which < 0 || which > 2) return fail(U1GF_EINVAL, "u1gf_set_kernel: bad argument");
     o->kernel_choice = which;
     return U1GF_OK;
 }
 
 static bool use_lanes(const u1gf_orbit* o) { return o->kernel_choice == 0 && lanes_supported(o); }
+static bool use_stream(const u1gf_orbit* o) {
+    if (use_lanes(o)) return false;
+    return (o->kernel_choice == 0 && stream_preferred(o)) || (o->kernel_choice == 2 && stream_supported(o));
+}
 
 const char* u1gf_kernel_name(const u1gf_orbit* o) {
     if (!o) return "";
-    return use_lanes(o) ? lanes_name(o) : "generic_cta_per_start";
+    return use_lanes(o) ? lanes_name(o) : use_stream(o) ? "stream_lane_per_start" : "generic_cta_per_start";
 }
 
 size_t u1gf_relax_workspace_bytes(const u1gf_orbit* o, uint64_t n_starts) {
     if (!o) return 0;
-    return use_lanes(o) ? lanes_workspace_bytes(o, n_starts) : generic_workspace_bytes(o, n_starts);
+    return use_lanes(o)    ? lanes_workspace_bytes(o, n_starts)
+           : use_stream(o) ? stream_workspace_bytes(o, n_starts)
+                           : generic_workspace_bytes(o, n_starts);
 }
 
 int u1gf_relax_batch(const u1gf_orbit* o, uint64_t seed, uint64_t first_start, uint64_t n_starts,
@@ -249,7 +255,7 @@ int u1gf_relax_batch(const u1gf_orbit* o, uint64_t seed, uint64_t first_start, u
         U1GF_CUDA(cudaEventCreate(&t_ev0));
         U1GF_CUDA(cudaEventCreate(&t_ev1));
     }
-    return use_lanes(o) ? lanes_relax(o, a, st) : generic_relax(o, a, st);
+    return use_lanes(o) ? lanes_relax(o, a, st) : use_stream(o) ? stream_relax(o, a, st) : generic_relax(o, a, st);
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -1,0 +1,408 @@
+// relax_stream.cu -- streamed "lane per start" relaxation kernel for the large even lattices (6^4, 8^4, ...).
+//
+// The resident kernels of relax_lanes.cu keep the gauge field of 32 starts in the registers of a team of warps; at
+// V = 1296 or 4096 sites that no longer fits on chip (32 starts x 64 KiB = 2 MiB).  Here the field of a team lives in
+// HBM / L2 in the layout [site][32 starts] (one 512-byte row per site, the start index fastest), and every half-sweep
+// streams the rows of the other parity through the SM:
+//   * lane l of every warp of the CTA works on start l of the team, so a neighbour is ONE coalesced 128-bit load of
+//     512 contiguous bytes per warp, and a link is one warp-uniform load shared by the 32 starts (the generic kernel
+//     pays 2d x 16 bytes of link traffic per site update, this one 2d x 16 / 32);
+//   * the warps of the CTA split the sites of the current parity; the CTA barrier between the half-sweeps is the
+//     only synchronisation (a team never leaves its SM, so its rows stay coherent through L1);
+//   * lane-level refill as in relax_lanes.cu: a start that stops is finalised (a5, a6) and replaced at once by the
+//     next start, both done by all threads of the CTA on that start's column of the team buffer.
+// Arithmetic of a site update and the stop rule (R5) are those of relax_lanes.cu / the oracle: sweep = even half-sweep,
+// odd half-sweep; odd-site Delta from the w just used, even-site Delta from the w formed at the start of the next
+// sweep; the even rows are double buffered (A[0], A[1]) so that the pre-update values survive the decision.
+#include "u1gf_internal.h"
+
+namespace u1gf {
+namespace {
+
+constexpr int kThreads = 512;
+constexpr int kWarps = kThreads / 32;
+
+struct StreamParams {
+    uint64_t seed, first_start, n_starts;
+    const uint64_t* start_ids;
+    double k2, eps;   // k2 = omega / (1 - omega) (unused when omega == 1)
+    int max_sweeps, check_every;
+    double* F_norm;
+    int32_t* sweeps;
+    uint8_t* status;
+    double* sig;
+    double* g_canon;
+    double2* team_buf;             // [teams][2][V][32]
+    unsigned long long* counter;   // next start position to hand out
+    OrbitDev D;
+};
+
+// sum over the CTA of NV per-thread values, same result in every thread, fixed order (deterministic)
+template <int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double (*red)[kWarps][NV], int& buf) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+        for (int q = 0; q < NV; ++q) v[q] += __shfl_down_sync(0xffffffffu, v[q], o);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0)
+#pragma unroll
+        for (int q = 0; q < NV; ++q) red[buf][warp][q] = v[q];
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < NV; ++q) {
+        double s = 0.0;
+        for (int w = 0; w < kWarps; ++w) s += red[buf][w][q];
+        v[q] = s;
+    }
+    buf ^= 1;
+}
+
+__device__ __noinline__ bool r6_vanishes(double nw) {
+    return (unsigned long long)__double_as_longlong(nw) < (unsigned long long)__double_as_longlong(1e-280);
+}
+
+// a3 for one site of one start: g <- normalise((1-omega) g + omega w/|w|) (R2) in the 8d+20 form of
+// relax_lanes.cu (h' = g + (k2/|w|) w = h/(1-omega), second-order rsqrt polish); W1: omega == 1, g <- w/|w|.
+template <bool W1>
+__device__ __forceinline__ double2 site_update(double2 g, double wr, double wi, double k2, bool& skipped) {
+    const double nw = fma(wr, wr, wi * wi);
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(nw));
+    const double e = fma(nw * y, -y, 1.0);
+    double2 gn;
+    if (W1) {
+        const double rs = fma(fma(e, 0.375, 0.5), y * e, y);
+        gn = make_double2(wr * rs, wi * rs);
+    } else {
+        const double c = fma(y * (0.5 * k2), e, y * k2);
+        const double hr = fma(c, wr, g.x), hi = fma(c, wi, g.y);
+        const double nh = fma(hr, hr, hi * hi);
+        double y2;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y2) : "d"(nh));
+        const double e2 = fma(nh * y2, -y2, 1.0);
+        const double r2 = fma(y2 * -0.5, e2, -y2);
+        gn = make_double2(hr * r2, hi * r2);
+    }
+    if (__double2hiint(nw) <= __double2hiint(1e-280)) {   // R6
+        if (r6_vanishes(nw)) {
+            gn = g;
+            skipped = true;
+        }
+    }
+    return gn;
+}
+
+template <int DIM>
+__device__ __forceinline__ int parity_of(const OrbitDev& D, int i) {
+    int p = 0;
+#pragma unroll
+    for (int mu = 0; mu < DIM; ++mu) {   // unrolled: constant indices keep the orbit descriptor in the constant bank
+        p += i % D.ext[mu];
+        i /= D.ext[mu];
+    }
+    return p & 1;
+}
+
+// Where the r-th site of parity p sits and who its neighbours are.  Tables: the orbit's order / fwd / bwd arrays (any
+// all-even lattice; three dependent global loads before the first row can be requested).  Cubic<N>: N^DIM lattices with
+// N a compile-time constant -- pure integer arithmetic, so the 2d rows and 2d links of a site are requested at once.
+template <int DIM>
+struct Tables {
+    __device__ static __forceinline__ void locate(const OrbitDev& D, int p, int r, int& i, int (&jf)[DIM], int (&jb)[DIM]) {
+        i = __ldg(D.order + p * D.phase_off[1] + r);
+#pragma unroll
+        for (int mu = 0; mu < DIM; ++mu) {
+            jf[mu] = __ldg(D.fwd + i * DIM + mu);
+            jb[mu] = __ldg(D.bwd + i * DIM + mu);
+        }
+    }
+};
+
+template <int DIM, int N>
+struct Cubic {
+    static_assert(N % 2 == 0, "even extent");
+    __device__ static __forceinline__ void locate(const OrbitDev&, int p, int r, int& i, int (&jf)[DIM], int (&jb)[DIM]) {
+        // sites 2r and 2r+1 differ in x0 only (N even), so exactly one of them has parity p
+        int x[DIM], rest = 2 * r, s = 0;
+#pragma unroll
+        for (int mu = 0; mu < DIM; ++mu) {
+            x[mu] = rest % N;
+            rest /= N;
+            if (mu > 0) s += x[mu];
+        }
+        const int f = ((s & 1) != p) ? 1 : 0;
+        x[0] += f;
+        i = 2 * r + f;
+        int stride = 1;
+#pragma unroll
+        for (int mu = 0; mu < DIM; ++mu) {
+            jf[mu] = i + (x[mu] == N - 1 ? -(N - 1) * stride : stride);
+            jb[mu] = i + (x[mu] == 0 ? (N - 1) * stride : -stride);
+            stride *= N;
+        }
+    }
+};
+
+// w_i = sum_mu [ conj(U_{i,mu}) g_{i+mu} + U_{i-mu,mu} g_{i-mu} ]   (= conj K_i of Eq. 5) for the start of
+// this lane; `nb` = rows of the other parity.  Link loads are warp-uniform (one sector each).
+template <int DIM>
+__device__ __forceinline__ void neighbour_sum(const OrbitDev& D, const double2* __restrict__ nb, int i, const int (&jf)[DIM],
+                                              const int (&jb)[DIM], int lane, double& wr, double& wi) {
+    double2 gf[DIM], gb[DIM];
+#pragma unroll
+    for (int mu = 0; mu < DIM; ++mu) {   // all 2d rows (L2 / HBM) in flight before the first FMA
+        gf[mu] = nb[(size_t)jf[mu] * 32 + lane];
+        gb[mu] = nb[(size_t)jb[mu] * 32 + lane];
+    }
+    wr = 0.0;
+    wi = 0.0;
+#pragma unroll
+    for (int mu = 0; mu < DIM; ++mu) {
+        const double2 uf = __ldg(D.U + i * DIM + mu);        // links: one sector per warp, mostly L1 hits
+        const double2 ub = __ldg(D.U + jb[mu] * DIM + mu);
+        wr = fma(uf.x, gf[mu].x, wr);
+        wi = fma(uf.x, gf[mu].y, wi);
+        wr = fma(uf.y, gf[mu].y, wr);
+        wi = fma(-uf.y, gf[mu].x, wi);
+        wr = fma(ub.x, gb[mu].x, wr);
+        wi = fma(ub.x, gb[mu].y, wi);
+        wr = fma(-ub.y, gb[mu].y, wr);
+        wi = fma(ub.y, gb[mu].x, wi);
+    }
+}
+
+template <int DIM, bool W1, class IDX>
+__global__ void __launch_bounds__(kThreads, 1) relax_stream_kernel(const StreamParams P) {
+    constexpr unsigned FULL = 0xffffffffu;
+    __shared__ double red[2][kWarps][5];
+    __shared__ double sred[2][kWarps][32];
+    __shared__ unsigned long long s_pos[32];
+    __shared__ unsigned s_skip[32];
+    __shared__ unsigned long long s_k;
+    const OrbitDev& D = P.D;
+    const int V = D.V, half = D.phase_off[1];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double2* const A0 = P.team_buf + (size_t)blockIdx.x * 2 * V * 32;
+    double2* const A1 = A0 + (size_t)V * 32;
+    auto rows = [&](int buf) { return buf ? A1 : A0; };
+
+    bool active = false, fresh = false, maxed = false, skipped = false;
+    int t = 0, eb = 0, rb = 0, fb = 0;
+    double accO = 0.0;
+    unsigned need = FULL, dumpm = 0;   // first pass: every lane needs a start, nothing to finalise
+
+    for (;;) {
+        // ---------------------------------------------------------- service (CTA-uniform): finalise, refill
+        for (unsigned m = need; m; m &= m - 1) {
+            const int L = __ffs(m) - 1;
+            if ((dumpm >> L) & 1u) {
+                // a5, a6 for the start of lane L: even rows before the last even half-sweep (A[eb]), odd rows A0
+                if (skipped) atomicOr(&s_skip[lane], 1u);
+                const int tL = __shfl_sync(FULL, t, L);
+                const int mxL = __shfl_sync(FULL, maxed ? 1 : 0, L);
+                const unsigned long long k = s_pos[L];
+                const double2* E = rows(eb);
+                const int pc = parity_of<DIM>(D, V - 1);
+                const double2 c = (pc ? A0 : E)[(size_t)(V - 1) * 32 + L];
+                double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+                for (int i = tid; i < V; i += kThreads) {
+                    const int pi = parity_of<DIM>(D, i);
+                    const double2 gi = (pi ? A0 : E)[(size_t)i * 32 + L];
+                    const double2* N = pi ? E : A0;   // neighbours have the other parity
+#pragma unroll
+                    for (int mu = 0; mu < DIM; ++mu) {   // F = sum Re(g_i U_{i,mu} conj g_{i+mu})   (Eq. 3)
+                        const double2 u = __ldg(D.U + i * DIM + mu);
+                        const double2 gj = N[(size_t)__ldg(D.fwd + i * DIM + mu) * 32 + L];
+                        const double ar = fma(gi.x, u.x, -gi.y * u.y), ai = fma(gi.x, u.y, gi.y * u.x);
+                        v[0] += fma(ar, gj.x, ai * gj.y);
+                    }
+                    const double re = fma(gi.x, c.x, gi.y * c.y);   // g~ = g conj(g_{V-1})
+                    const double im = fma(gi.y, c.x, -gi.x * c.y);
+                    const unsigned bits = __ldg(D.sgn + i);
+                    v[1] += ((bits & 1u) ? re : -re) + ((bits & 16u) ? im : -im);
+                    v[2] += ((bits & 2u) ? re : -re) + ((bits & 32u) ? im : -im);
+                    v[3] += ((bits & 4u) ? re : -re) + ((bits & 64u) ? im : -im);
+                    v[4] += ((bits & 8u) ? re : -re) + ((bits & 128u) ? im : -im);
+                    if (P.g_canon) reinterpret_cast<double2*>(P.g_canon)[k * (unsigned long long)V + i] = make_double2(re, im);
+                }
+                block_sum<5>(v, red, fb);   // its barrier also publishes the s_skip bits
+                if (tid == 0) {
+                    P.F_norm[k] = v[0] / ((double)DIM * (double)V);
+                    P.sweeps[k] = tL;
+                    P.status[k] = (uint8_t)((mxL ? 1 : 0) | (s_skip[L] ? 2 : 0));
+                    reinterpret_cast<double4*>(P.sig)[k] =
+                        make_double4(v[1] / (double)V, v[2] / (double)V, v[3] / (double)V, v[4] / (double)V);
+                }
+            }
+            // the next start for lane L
+            if (tid == 0) s_k = atomicAdd(P.counter, 1ull);
+            __syncthreads();
+            const unsigned long long k = s_k;
+            if (k < P.n_starts) {
+                const uint64_t s = P.start_ids ? P.start_ids[k] : P.first_start + k;
+                double2* En = rows(eb ^ 1);   // where the next even half-sweep looks for its own sites
+                for (int i = tid; i < V; i += kThreads) {   // a2: Philox counter (site, start lo, start hi, 0)
+                    const u32x4 r = philox((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 0u, (uint32_t)P.seed,
+                                           (uint32_t)(P.seed >> 32));
+                    double sn, cs;
+                    sincospi(unit_interval_pm1(r.x, r.y), &sn, &cs);
+                    (parity_of<DIM>(D, i) ? A0 : En)[(size_t)i * 32 + L] = make_double2(cs, sn);
+                }
+                if (tid == 0) {
+                    s_pos[L] = k;
+                    s_skip[L] = 0u;
+                }
+                if (lane == L) {
+                    active = true;
+                    fresh = true;   // a new start begins with its even half-sweep
+                    t = 0;
+                    skipped = false;
+                }
+            } else if (lane == L) {
+                active = false;
+            }
+            __syncthreads();
+        }
+        if (__ballot_sync(FULL, active) == 0) break;   // every warp holds the same lane states
+
+        // ---------------------------------------------------------- odd half-sweep (second half of sweep t+1)
+        {
+            const bool commit = active && !fresh;
+            const double2* E = rows(eb ^ 1);   // the values written by the last even half-sweep
+            accO = 0.0;
+            for (int r = warp; r < half; r += kWarps) {
+                int i, jf[DIM], jb[DIM];
+                IDX::locate(D, 1, r, i, jf, jb);
+                double wr, wi;
+                neighbour_sum<DIM>(D, E, i, jf, jb, lane, wr, wi);
+                double2* own = A0 + (size_t)i * 32 + lane;
+                bool sk = false;
+                const double2 gn = site_update<W1>(*own, wr, wi, P.k2, sk);
+                if (commit) {
+                    *own = gn;
+                    const double dl = fma(gn.y, wr, -gn.x * wi);   // Delta_i = Im(g_i conj w_i) after the update
+                    accO = fma(dl, dl, accO);
+                    skipped |= sk;
+                }
+            }
+            if (commit) ++t;
+            fresh = false;
+            eb ^= 1;
+        }
+        __syncthreads();
+
+        // ---------------------------------------------------------- even half-sweep (first half of sweep t+1)
+        double accE = 0.0;
+        {
+            const double2* E = rows(eb);
+            double2* En = rows(eb ^ 1);
+            for (int r = warp; r < half; r += kWarps) {
+                int i, jf[DIM], jb[DIM];
+                IDX::locate(D, 0, r, i, jf, jb);
+                double wr, wi;
+                neighbour_sum<DIM>(D, A0, i, jf, jb, lane, wr, wi);
+                const double2 g = E[(size_t)i * 32 + lane];
+                const double dl = fma(g.y, wr, -g.x * wi);   // Delta_i of the field after sweep t
+                accE = fma(dl, dl, accE);
+                bool sk = false;
+                const double2 gn = site_update<W1>(g, wr, wi, P.k2, sk);
+                if (active) {
+                    En[(size_t)i * 32 + lane] = gn;
+                    skipped |= sk;
+                }
+            }
+        }
+        // a4: gauge precision of the field after sweep t (R5), fixed summation order over the warps
+        sred[rb][warp][lane] = accE + accO;
+        __syncthreads();
+        double S = 0.0;
+#pragma unroll
+        for (int w = 0; w < kWarps; ++w) S += sred[rb][w][lane];
+        rb ^= 1;
+        const bool conv = active && t > 0 && (t % P.check_every == 0) && (S / (double)V < P.eps);
+        maxed = active && !conv && t == P.max_sweeps;
+        dumpm = __ballot_sync(FULL, conv || maxed);
+        need = dumpm;
+    }
+}
+
+template <int DIM, bool W1, class IDX>
+int launch_k(const u1gf_orbit* o, const RelaxArgs& a, StreamParams& P, cudaStream_t st) {
+    auto kern = relax_stream_kernel<DIM, W1, IDX>;
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kThreads, 0) != cudaSuccess) per_sm = 0;
+    unsigned long long teams = (unsigned long long)per_sm * (unsigned long long)o->sm_count;
+    const unsigned long long batches = (a.n_starts + 31) / 32;
+    if (teams > batches) teams = batches;
+    if (teams > 2ull * (unsigned long long)o->sm_count) teams = 2ull * (unsigned long long)o->sm_count;   // workspace bound
+    if (teams < 1) return fail(U1GF_ECUDA, "streamed relaxation kernel does not fit on an SM");
+    // counter and team buffers start from zero (an idle lane then reads a null field, not stale bits)
+    const size_t bytes = 256 + (size_t)teams * 2 * (size_t)o->dev.V * 32 * sizeof(double2);
+    U1GF_CUDA(cudaMemsetAsync(a.workspace, 0, bytes, st));
+    U1GF_CUDA(cudaEventRecord(t_ev0, st));
+    kern<<<(unsigned)teams, kThreads, 0, st>>>(P);
+    U1GF_CUDA(cudaGetLastError());
+    U1GF_CUDA(cudaEventRecord(t_ev1, st));
+    t_ev_valid = true;
+    ++t_launches;
+    return U1GF_OK;
+}
+
+template <int DIM, class IDX>
+int launch_w(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st) {
+    const bool w1 = a.omega == 1.0;
+    StreamParams P;
+    P.seed = a.seed; P.first_start = a.first_start; P.n_starts = a.n_starts; P.start_ids = a.start_ids;
+    P.k2 = w1 ? 0.0 : a.omega / (1.0 - a.omega); P.eps = a.eps;
+    P.max_sweeps = a.max_sweeps; P.check_every = a.check_every;
+    P.F_norm = a.F_norm; P.sweeps = a.sweeps; P.status = a.status; P.sig = a.sig; P.g_canon = a.g_canon;
+    P.counter = (unsigned long long*)a.workspace;
+    P.team_buf = (double2*)((char*)a.workspace + 256);
+    P.D = o->dev;
+    return w1 ? launch_k<DIM, true, IDX>(o, a, P, st) : launch_k<DIM, false, IDX>(o, a, P, st);
+}
+
+template <int DIM>
+bool cubic(const u1gf_orbit* o, int n) {
+    for (int mu = 0; mu < DIM; ++mu)
+        if (o->dev.ext[mu] != n) return false;
+    return true;
+}
+
+template <int DIM>
+int launch(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st) {
+    if (DIM >= 2) {
+        if (cubic<DIM>(o, 6)) return launch_w<DIM, Cubic<DIM, 6>>(o, a, st);
+        if (cubic<DIM>(o, 8)) return launch_w<DIM, Cubic<DIM, 8>>(o, a, st);
+        if (DIM <= 3 && cubic<DIM>(o, 10)) return launch_w<DIM, Cubic<DIM, 10>>(o, a, st);
+    }
+    return launch_w<DIM, Tables<DIM>>(o, a, st);
+}
+
+}  // namespace
+
+// every extent even (two-colour checkerboard); chosen automatically from 512 sites up, where a team's field no longer
+// fits on chip and the generic kernel's per-start link traffic dominates
+bool stream_supported(const u1gf_orbit* o) { return o->dev.all_even && o->dev.d >= 1 && o->dev.d <= 4; }
+bool stream_preferred(const u1gf_orbit* o) { return stream_supported(o) && o->dev.V >= 512; }
+
+size_t stream_workspace_bytes(const u1gf_orbit* o, uint64_t n) {
+    // upper bound on the teams of a launch: 2 CTAs per SM, never more than the batches of 32 starts
+    unsigned long long teams = 2ull * (unsigned long long)o->sm_count;
+    const unsigned long long batches = (n + 31) / 32;
+    if (teams > batches) teams = batches;
+    if (teams < 1) teams = 1;
+    return 256 + (size_t)teams * 2 * (size_t)o->dev.V * 32 * sizeof(double2);
+}
+
+int stream_relax(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st) {
+    switch (o->dev.d) {
+        case 1: return launch<1>(o, a, st);
+        case 2: return launch<2>(o, a, st);
+        case 3: return launch<3>(o, a, st);
+        default: return launch<4>(o, a, st);
+    }
+}
+
+}  // namespace u1gf

@@ -106,7 +106,7 @@ struct u1gf_orbit {
     size_t blob_bytes = 0;
     int device = 0;
     int sm_count = 0;
-    int kernel_choice = 0;  // 0 auto, 1 generic
+    int kernel_choice = 0;  // 0 auto, 1 generic, 2 streamed (falls back to generic where it does not apply)
     // device copy of the links in the layout of the specialised resident kernels (inside blob), or null
     const double2* U_lanes = nullptr;
 };
@@ -138,5 +138,11 @@ size_t lanes_links_bytes(int d, const int* ext);  // extra blob bytes for the ke
 void lanes_fill_links(int d, const int* ext, const double* U_host, double2* dst_host);
 size_t lanes_workspace_bytes(const u1gf_orbit* o, uint64_t n);
 int lanes_relax(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st);
+
+// streamed "lane per start" kernel for the large even lattices (relax_stream.cu)
+bool stream_supported(const u1gf_orbit* o);   // every extent even
+bool stream_preferred(const u1gf_orbit* o);   // ... and large enough to be the automatic choice
+size_t stream_workspace_bytes(const u1gf_orbit* o, uint64_t n);
+int stream_relax(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st);
 
 }  // namespace u1gf

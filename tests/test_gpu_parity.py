@@ -48,19 +48,29 @@ LATTICES = [
     ((4, 4), 1, 512), ((8, 8), 2, 256), ((4, 4, 4), 3, 256), ((4, 4, 4, 4), 12, 96), ((2, 2, 2, 2), 12, 512),
     ((3, 3, 3, 3), 12, 128), ((3, 2), 40, 256), ((2, 2), 41, 256), ((5, 3, 2), 7, 128), ((6, 6, 6, 6), 12, 12),
     ((8, 8, 8, 8), 12, 4), ((7,), 77, 128), ((6, 4), 5, 128), ((4, 6, 2, 3), 9, 32), ((10, 10), 8, 64),
+    ((8, 8, 8), 21, 70), ((6, 6), 22, 300),
 ]
 
 
 @pytest.mark.parametrize("ext,seed,n", LATTICES)
-@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("kernel", [0, 1, 2])
 def test_relax_matches_oracle(b, oracle, ext, seed, n, kernel):
-    """a2-a6 on hot orbits: every lattice shape the kernels dispatch on (resident specialisations, generic even,
-    generic odd-extent level phases, extent-2 double bonds, d = 1), both the automatic and the generic kernel."""
+    """a2-a6 on hot orbits: every lattice shape the kernels dispatch on (resident specialisations, streamed large even
+    lattices, generic even, generic odd-extent level phases, extent-2 double bonds, d = 1): the automatic choice, the
+    generic kernel, and the streamed kernel forced onto every all-even lattice (refill and ragged teams included:
+    n is not a multiple of 32 for some of them)."""
     th = synth.uniform_links(ext, seed)
     orbit = b.Orbit(ext, th)
     orbit.set_kernel(kernel)
     if kernel == 1 and orbit.kernel_name != "generic_cta_per_start":
         pytest.fail("set_kernel(1) must select the generic kernel")
+    if kernel == 2:
+        if any(e % 2 for e in ext):
+            pytest.skip("the streamed kernel needs even extents")
+        if orbit.kernel_name != "stream_lane_per_start":
+            pytest.fail("set_kernel(2) must select the streamed kernel on an all-even lattice")
+    if kernel == 0 and orbit.V >= 512 and not any(e % 2 for e in ext):
+        assert orbit.kernel_name == "stream_lane_per_start"
     V = orbit.V
     eps = 1e-12 if V > 256 else 1e-13
     o = oracle.relax(ext, th, seed, n, eps=eps, want_g=True)
