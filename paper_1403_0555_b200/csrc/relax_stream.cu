@@ -21,6 +21,10 @@ namespace {
 
 constexpr int kThreads = 512;
 constexpr int kWarps = kThreads / 32;
+#ifndef U1GF_STREAM_AHEAD
+#define U1GF_STREAM_AHEAD 0
+#endif
+constexpr int kPrefetchAhead = U1GF_STREAM_AHEAD;   // sites of this warp between a prefetch and its use
 
 struct StreamParams {
     uint64_t seed, first_start, n_starts;
@@ -109,6 +113,7 @@ __device__ __forceinline__ int parity_of(const OrbitDev& D, int i) {
 // N a compile-time constant -- pure integer arithmetic, so the 2d rows and 2d links of a site are requested at once.
 template <int DIM>
 struct Tables {
+    static constexpr bool kPrefetch = false;   // locating a site costs dependent loads here
     __device__ static __forceinline__ void locate(const OrbitDev& D, int p, int r, int& i, int (&jf)[DIM], int (&jb)[DIM]) {
         i = __ldg(D.order + p * D.phase_off[1] + r);
 #pragma unroll
@@ -121,6 +126,7 @@ struct Tables {
 
 template <int DIM, int N>
 struct Cubic {
+    static constexpr bool kPrefetch = true;
     static_assert(N % 2 == 0, "even extent");
     __device__ static __forceinline__ void locate(const OrbitDev&, int p, int r, int& i, int (&jf)[DIM], int (&jb)[DIM]) {
         // sites 2r and 2r+1 differ in x0 only (N even), so exactly one of them has parity p
@@ -149,9 +155,16 @@ struct Cubic {
 template <int DIM>
 __device__ __forceinline__ void neighbour_sum(const OrbitDev& D, const double2* __restrict__ nb, int i, const int (&jf)[DIM],
                                               const int (&jb)[DIM], int lane, double& wr, double& wi) {
-    double2 gf[DIM], gb[DIM];
+    // all 2d links and 2d rows in flight before the first FMA (ncu: with the link loads left inside the FMA loop,
+    // 46 % of the warp time sat on the long scoreboard of the second FMA -- the links miss L1, the rows evict them)
+    double2 gf[DIM], gb[DIM], uf[DIM], ub[DIM];
 #pragma unroll
-    for (int mu = 0; mu < DIM; ++mu) {   // all 2d rows (L2 / HBM) in flight before the first FMA
+    for (int mu = 0; mu < DIM; ++mu) {
+        uf[mu] = __ldg(D.U + i * DIM + mu);
+        ub[mu] = __ldg(D.U + jb[mu] * DIM + mu);
+    }
+#pragma unroll
+    for (int mu = 0; mu < DIM; ++mu) {
         gf[mu] = nb[(size_t)jf[mu] * 32 + lane];
         gb[mu] = nb[(size_t)jb[mu] * 32 + lane];
     }
@@ -159,17 +172,29 @@ __device__ __forceinline__ void neighbour_sum(const OrbitDev& D, const double2* 
     wi = 0.0;
 #pragma unroll
     for (int mu = 0; mu < DIM; ++mu) {
-        const double2 uf = __ldg(D.U + i * DIM + mu);        // links: one sector per warp, mostly L1 hits
-        const double2 ub = __ldg(D.U + jb[mu] * DIM + mu);
-        wr = fma(uf.x, gf[mu].x, wr);
-        wi = fma(uf.x, gf[mu].y, wi);
-        wr = fma(uf.y, gf[mu].y, wr);
-        wi = fma(-uf.y, gf[mu].x, wi);
-        wr = fma(ub.x, gb[mu].x, wr);
-        wi = fma(ub.x, gb[mu].y, wi);
-        wr = fma(-ub.y, gb[mu].y, wr);
-        wi = fma(ub.y, gb[mu].x, wi);
+        wr = fma(uf[mu].x, gf[mu].x, wr);
+        wi = fma(uf[mu].x, gf[mu].y, wi);
+        wr = fma(uf[mu].y, gf[mu].y, wr);
+        wi = fma(-uf[mu].y, gf[mu].x, wi);
+        wr = fma(ub[mu].x, gb[mu].x, wr);
+        wi = fma(ub[mu].x, gb[mu].y, wi);
+        wr = fma(-ub[mu].y, gb[mu].y, wr);
+        wi = fma(ub[mu].y, gb[mu].x, wi);
     }
+}
+
+// Request the rows the NEXT site of this warp will read (its 2d neighbours and itself) into L1 while the current
+// site is computed: the half-sweep is otherwise bound by the L2 / HBM latency of one site per warp (ncu: long
+// scoreboard 5.8 stalled warps per issue).  Costs no registers; every lane touches its own 16 bytes of the row.
+template <int DIM>
+__device__ __forceinline__ void prefetch_rows(const double2* nb, const double2* own, int i, const int (&jf)[DIM],
+                                              const int (&jb)[DIM], int lane) {
+#pragma unroll
+    for (int mu = 0; mu < DIM; ++mu) {
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(nb + (size_t)jf[mu] * 32 + lane));
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(nb + (size_t)jb[mu] * 32 + lane));
+    }
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(own + (size_t)i * 32 + lane));
 }
 
 template <int DIM, bool W1, class IDX>
@@ -273,14 +298,19 @@ __global__ void __launch_bounds__(kThreads, 1) relax_stream_kernel(const StreamP
             accO = 0.0;
             for (int r = warp; r < half; r += kWarps) {
                 int i, jf[DIM], jb[DIM];
+                if (IDX::kPrefetch && kPrefetchAhead > 0 && r + kPrefetchAhead * kWarps < half) {
+                    IDX::locate(D, 1, r + kPrefetchAhead * kWarps, i, jf, jb);
+                    prefetch_rows<DIM>(E, A0, i, jf, jb, lane);
+                }
                 IDX::locate(D, 1, r, i, jf, jb);
                 double wr, wi;
                 neighbour_sum<DIM>(D, E, i, jf, jb, lane, wr, wi);
                 double2* own = A0 + (size_t)i * 32 + lane;
                 bool sk = false;
-                const double2 gn = site_update<W1>(*own, wr, wi, P.k2, sk);
+                // own rows are read and written once per half-sweep: streaming hints keep L1 for the neighbour rows
+                const double2 gn = site_update<W1>(__ldcs(own), wr, wi, P.k2, sk);
                 if (commit) {
-                    *own = gn;
+                    __stcs(own, gn);
                     const double dl = fma(gn.y, wr, -gn.x * wi);   // Delta_i = Im(g_i conj w_i) after the update
                     accO = fma(dl, dl, accO);
                     skipped |= sk;
@@ -299,16 +329,20 @@ __global__ void __launch_bounds__(kThreads, 1) relax_stream_kernel(const StreamP
             double2* En = rows(eb ^ 1);
             for (int r = warp; r < half; r += kWarps) {
                 int i, jf[DIM], jb[DIM];
+                if (IDX::kPrefetch && kPrefetchAhead > 0 && r + kPrefetchAhead * kWarps < half) {
+                    IDX::locate(D, 0, r + kPrefetchAhead * kWarps, i, jf, jb);
+                    prefetch_rows<DIM>(A0, E, i, jf, jb, lane);
+                }
                 IDX::locate(D, 0, r, i, jf, jb);
                 double wr, wi;
                 neighbour_sum<DIM>(D, A0, i, jf, jb, lane, wr, wi);
-                const double2 g = E[(size_t)i * 32 + lane];
+                const double2 g = __ldcs(E + (size_t)i * 32 + lane);
                 const double dl = fma(g.y, wr, -g.x * wi);   // Delta_i of the field after sweep t
                 accE = fma(dl, dl, accE);
                 bool sk = false;
                 const double2 gn = site_update<W1>(g, wr, wi, P.k2, sk);
                 if (active) {
-                    En[(size_t)i * 32 + lane] = gn;
+                    __stcs(En + (size_t)i * 32 + lane, gn);
                     skipped |= sk;
                 }
             }
@@ -330,6 +364,7 @@ __global__ void __launch_bounds__(kThreads, 1) relax_stream_kernel(const StreamP
 template <int DIM, bool W1, class IDX>
 int launch_k(const u1gf_orbit* o, const RelaxArgs& a, StreamParams& P, cudaStream_t st) {
     auto kern = relax_stream_kernel<DIM, W1, IDX>;
+    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 5);   // percent: the rest is L1 for the rows
     int per_sm = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kThreads, 0) != cudaSuccess) per_sm = 0;
     unsigned long long teams = (unsigned long long)per_sm * (unsigned long long)o->sm_count;
