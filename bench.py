@@ -260,7 +260,23 @@ def main():
                 "note": ("achieved = site-updates x (8d+16 = %d algorithmic FP64 instructions) x 2 flop / kernel time; "
                          "peak = 2 x DFMA/s of the in-run u1gf_measure_fp64_peak microbenchmark (kernel timed alone; constant "
                          "multiplicands); dfma_rate_* = the same unit for DFMA streams with register multiplicands, "
-                         "which the register file limits to 2/3 of peak (DESIGN.md section 7)") % A_D[d]}
+                         "which the register file limits to 3/4 of peak (DESIGN.md section 7.1)") % A_D[d]}
+    if orbit.kernel_name.startswith("stream"):
+        # the streamed kernel (large lattices) is bound by memory traffic: algorithmic bytes = one read and one write of
+        # g per site update (32 B); peak = the driver's measured HBM copy bandwidth
+        hbm_peak, how = 6650.0, "fallback of B200_PROFILING.md"
+        try:
+            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+                hbm_peak, how = float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json"
+        except (OSError, KeyError, ValueError):
+            pass
+        gbs = per_rank_su * 32.0 / (k_ms * 1e-3) / 1e9 if k_ms else None
+        roofline = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
+                    "frac": gbs / hbm_peak if gbs else None, "traffic": None, "peak_source": how,
+                    "fp64_frac": roofline["frac"], "kernel": orbit.kernel_name, "kernel_ms": k_ms,
+                    "kernel_share_of_step": k_ms / ms_per_step if k_ms else None,
+                    "note": "achieved = site-updates x 32 algorithmic bytes / kernel time; fp64_frac = the same launch "
+                            "against the measured FP64 peak (A_d algorithmic instructions per site update)"}
     cpu = None
     if not args.no_cpu_baseline:
         cpu, _, _ = oracle_leg(conf, ob, 10.0)
