@@ -57,26 +57,42 @@ __device__ __forceinline__ void block_sum2(double& a, double& b, double (*red)[3
     buf ^= 1;
 }
 
-// number of eigenvalues of the k x k tridiagonal (alpha[0..k), beta[0..k-1)) below x (Sturm sequence)
-__device__ __forceinline__ int sturm_count(const double* alpha, const double* beta, int k, double x) {
-    int cnt = 0;
-    double q = alpha[0] - x;
-    if (q < 0.0) ++cnt;
+// power of two that brings |p| back near 1 (0 and denormals: no scaling)
+__device__ __forceinline__ double unit_scale(double p) {
+    const int e = (__double2hiint(p) >> 20) & 0x7ff;
+    return e == 0 ? 1.0 : __hiloint2double((2046 - e) << 20, 0);
+}
+
+// Number of eigenvalues of the k x k tridiagonal T_k (alpha[0..k), off-diagonal squares beta2[0..k-1)) below x: sign
+// changes of the leading principal minors p_j = det(T_j - x), p_j = (alpha_j - x) p_{j-1} - beta_{j-1}^2 p_{j-2}.
+// Division free (the pivot form q_j = p_j / p_{j-1} costs an FP64 division per step in a dependent chain); the pair
+// is rescaled every 8 steps.
+__device__ __forceinline__ int sturm_count(const double* alpha, const double* beta2, int k, double x) {
+    double p0 = 1.0, p1 = alpha[0] - x;
+    if (p1 == 0.0) p1 = 1e-300;
+    int cnt = p1 < 0.0 ? 1 : 0;
     for (int j = 1; j < k; ++j) {
-        if (fabs(q) < 1e-300) q = 1e-300;
-        q = alpha[j] - x - beta[j - 1] * beta[j - 1] / q;
-        if (q < 0.0) ++cnt;
+        double p2 = fma(alpha[j] - x, p1, -beta2[j - 1] * p0);
+        if (p2 == 0.0) p2 = p1 * 1e-300;   // a vanishing minor takes the sign of its predecessor: no change
+        cnt += ((p2 < 0.0) != (p1 < 0.0)) ? 1 : 0;
+        p0 = p1;
+        p1 = p2;
+        if ((j & 7) == 7) {
+            const double sc = unit_scale(p1);
+            p0 *= sc;
+            p1 *= sc;
+        }
     }
     return cnt;
 }
 
 // Smallest eigenvalue of T_k by 33-way multisection on warp 0 (all 32 lanes call this), bracket [lo, hi].
-__device__ double smallest_ritz(const double* alpha, const double* beta, int k, double lo, double hi) {
+__device__ double smallest_ritz(const double* alpha, const double* beta2, int k, double lo, double hi) {
     const int lane = threadIdx.x & 31;
     for (int it = 0; it < 14; ++it) {
         const double h = (hi - lo) / 33.0;
         const double x = lo + h * (double)(lane + 1);
-        const int c = sturm_count(alpha, beta, k, x);
+        const int c = sturm_count(alpha, beta2, k, x);
         const unsigned m = __ballot_sync(0xffffffffu, c >= 1);
         if (m == 0) {
             lo = lo + h * 32.0;
@@ -90,22 +106,27 @@ __device__ double smallest_ritz(const double* alpha, const double* beta, int k, 
     return 0.5 * (lo + hi);
 }
 
-// |last component| of the normalised eigenvector of T_k for (an approximation from below of) its smallest
-// eigenvalue: s_{j+1} = -(q_j/beta_j) s_j with the Sturm quotients q_j.
-__device__ double last_component(const double* alpha, const double* beta, int k, double lam) {
-    double q = alpha[0] - lam, s = 1.0, norm2 = 1.0;
-    for (int j = 1; j < k; ++j) {
-        if (fabs(q) < 1e-300) q = 1e-300;
-        const double r = -q / beta[j - 1];
-        s *= r;
-        norm2 = fma(s, s, norm2);
+// |last component| of the normalised eigenvector of T_k for (an approximation of) its smallest eigenvalue.  The
+// components of that vector DECAY towards the end -- that decay is the convergence of the Ritz value -- so the
+// three-term recurrence is run backwards from x_{k-1} = 1, the direction in which the wanted solution grows and
+// rounding errors do not: x_{j-1} = ((lam - alpha_j) x_j - beta_j x_{j+1}) / beta_{j-1}.  (Run forwards it stalls
+// near 1e-8, the stop test never fires and every configuration takes the maximum number of steps.)
+__device__ double last_component(const double* alpha, const double* beta, const double* ibeta, int k, double lam) {
+    double xn = 0.0, xc = 1.0, norm2 = 1.0, last = 1.0;   // x_{j+1}, x_j; `last` follows the scale of x_{k-1}
+    for (int j = k - 1; j >= 1; --j) {
+        const double bnext = j + 1 < k ? beta[j] : 0.0;
+        double xp = fma(lam - alpha[j], xc, -bnext * xn) * ibeta[j - 1];
+        norm2 = fma(xp, xp, norm2);
         if (norm2 > 1e200) {  // rescale
-            s *= 1e-100;
+            xc *= 1e-100;
+            xp *= 1e-100;
+            last *= 1e-100;
             norm2 *= 1e-200;
         }
-        q = alpha[j] - lam - beta[j - 1] * beta[j - 1] / q;
+        xn = xc;
+        xc = xp;
     }
-    return fabs(s) * rsqrt(norm2);
+    return fabs(last) * rsqrt(norm2);
 }
 
 template <int DIM>
@@ -116,7 +137,7 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
     double* va = c + (size_t)V * DIM;  // [V]
     double* vb = va + V;            // [V]
     __shared__ double red[2][32], red2[2][32];
-    __shared__ double alpha[kMaxK], beta[kMaxK];
+    __shared__ double alpha[kMaxK], beta[kMaxK], beta2[kMaxK], ibeta[kMaxK];
     __shared__ double s_lam, s_res;
     int buf = 0;
     const int kmax = min(V - 1, kMaxK);
@@ -194,14 +215,16 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
             if (tid == 0) {
                 alpha[k] = a;
                 beta[k] = b;
+                beta2[k] = sww;
+                ibeta[k] = 1.0 / b;
             }
             ++k;
             const bool breakdown = b < 1e-13 * (4.0 * DIM);
             if (breakdown || k == kmax || k == next_check) {
                 __syncthreads();
                 if (tid < 32) {
-                    const double l = smallest_ritz(alpha, beta, k, -(4.0 * DIM + 1.0), lam_hi);
-                    const double res = breakdown ? 0.0 : b * last_component(alpha, beta, k, l - 1e-13);
+                    const double l = smallest_ritz(alpha, beta2, k, -(4.0 * DIM + 1.0), lam_hi);
+                    const double res = breakdown ? 0.0 : b * last_component(alpha, beta, ibeta, k, l - 1e-13);
                     if (tid == 0) {
                         s_lam = l;
                         s_res = res;
@@ -226,7 +249,11 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
         if (tid == 0) {
             P.lambda1[cfg] = lam;
             const uint8_t reg = lam > P.tol_fp ? 1 : (fabs(lam) <= P.tol_fp ? 2 : 0);
+#ifdef U1GF_FP_DEBUG_K
+            P.region[cfg] = (uint8_t)min(k, 255);
+#else
             P.region[cfg] = reg;
+#endif
             if (reg) atomicAdd(P.n_in, 1ull);
         }
     }
