@@ -114,6 +114,7 @@ __device__ __forceinline__ int parity_of(const OrbitDev& D, int i) {
 template <int DIM>
 struct Tables {
     static constexpr bool kPrefetch = false;   // locating a site costs dependent loads here
+    static constexpr int kBlocksN = 0;         // no block-wise half-sweep
     __device__ static __forceinline__ void locate(const OrbitDev& D, int p, int r, int& i, int (&jf)[DIM], int (&jb)[DIM]) {
         i = __ldg(D.order + p * D.phase_off[1] + r);
 #pragma unroll
@@ -127,6 +128,7 @@ struct Tables {
 template <int DIM, int N>
 struct Cubic {
     static constexpr bool kPrefetch = true;
+    static constexpr int kBlocksN = N;   // extent for the block-wise half-sweep
     static_assert(N % 2 == 0, "even extent");
     __device__ static __forceinline__ void locate(const OrbitDev&, int p, int r, int& i, int (&jf)[DIM], int (&jb)[DIM]) {
         // sites 2r and 2r+1 differ in x0 only (N even), so exactly one of them has parity p
@@ -181,6 +183,101 @@ __device__ __forceinline__ void neighbour_sum(const OrbitDev& D, const double2* 
         wr = fma(-ub[mu].y, gb[mu].y, wr);
         wi = fma(ub[mu].y, gb[mu].x, wi);
     }
+}
+
+// Half-sweep of parity PAR over the 2^DIM blocks of an N^DIM lattice that warp `warp` owns (blocks warp, warp+16, ...).
+// The 2^(DIM-1) sites of the other parity inside a block are loaded once into registers and serve DIM of the 2 DIM
+// neighbours of each of the block's sites (as in the resident kernels); the other DIM neighbours, the site itself and
+// the links come from L1 / L2.  Per site: DIM + 1 + 1/.. row loads instead of 2 DIM + 1.
+//   src / dst  rows holding the parity-PAR sites before / after the update (the same array for the odd half-sweep)
+//   oth        rows of the other parity
+// Returns sum Delta_i^2 of this warp's sites for the lane's start: PAR == 0 measured before the update, 1 after it.
+template <int DIM, int N, int PAR, bool W1>
+__device__ __forceinline__ double half_sweep_blocks(const OrbitDev& D, const double2* src, double2* dst, const double2* oth,
+                                                    int warp, int lane, double k2, bool commit, bool& skipped) {
+    constexpr int NB1 = N / 2, HB = 1 << (DIM - 1);
+    int nblk = 1;
+#pragma unroll
+    for (int mu = 0; mu < DIM; ++mu) nblk *= NB1;
+    double acc = 0.0;
+    for (int b = warp; b < nblk; b += kWarps) {
+        int o[DIM], base = 0, rest = b, stride = 1;
+#pragma unroll
+        for (int mu = 0; mu < DIM; ++mu) {
+            o[mu] = 2 * (rest % NB1);
+            rest /= NB1;
+            base += o[mu] * stride;
+            stride *= N;
+        }
+        // local site l (one bit per direction) sits at base + off(l); parity of l = popc(l) (block origins are even)
+        auto off = [](int l) {
+            int r = 0, st = 1;
+#pragma unroll
+            for (int mu = 0; mu < DIM; ++mu) {
+                r += ((l >> mu) & 1) * st;
+                st *= N;
+            }
+            return r;
+        };
+        double2 in[HB];   // the block's sites of the other parity, by half index l >> 1
+#pragma unroll
+        for (int h = 0; h < HB; ++h) {
+            const int l = 2 * h + (((__popc(h) & 1) != (1 - PAR)) ? 1 : 0);
+            in[h] = oth[(size_t)(base + off(l)) * 32 + lane];
+        }
+#pragma unroll
+        for (int h = 0; h < HB; ++h) {
+            const int l = 2 * h + (((__popc(h) & 1) != PAR) ? 1 : 0);
+            const int i = base + off(l);
+            const double2 g = __ldcs(src + (size_t)i * 32 + lane);
+            double2 gf[DIM], gb[DIM], uf[DIM], ub[DIM];
+            int st = 1;
+#pragma unroll
+            for (int mu = 0; mu < DIM; ++mu) {
+                const int ln = l ^ (1 << mu);   // the in-block neighbour along mu
+                if (((l >> mu) & 1) == 0) {     // forward neighbour inside, backward one outside (periodic)
+                    const int jb = (o[mu] == 0) ? i + (N - 1) * st : i - st;
+                    gf[mu] = in[ln >> 1];
+                    gb[mu] = oth[(size_t)jb * 32 + lane];
+                    ub[mu] = __ldg(D.U + jb * DIM + mu);
+                } else {                        // backward neighbour inside, forward one outside (periodic)
+                    const int jf = (o[mu] + 2 == N) ? i + st - N * st : i + st;
+                    gf[mu] = oth[(size_t)jf * 32 + lane];
+                    gb[mu] = in[ln >> 1];
+                    ub[mu] = __ldg(D.U + (i - st) * DIM + mu);
+                }
+                uf[mu] = __ldg(D.U + i * DIM + mu);
+                st *= N;
+            }
+            double wr = 0.0, wi = 0.0;
+#pragma unroll
+            for (int mu = 0; mu < DIM; ++mu) {   // w_i (= conj K_i of Eq. 5)
+                wr = fma(uf[mu].x, gf[mu].x, wr);
+                wi = fma(uf[mu].x, gf[mu].y, wi);
+                wr = fma(uf[mu].y, gf[mu].y, wr);
+                wi = fma(-uf[mu].y, gf[mu].x, wi);
+                wr = fma(ub[mu].x, gb[mu].x, wr);
+                wi = fma(ub[mu].x, gb[mu].y, wi);
+                wr = fma(-ub[mu].y, gb[mu].y, wr);
+                wi = fma(ub[mu].y, gb[mu].x, wi);
+            }
+            if (PAR == 0) {
+                const double dl = fma(g.y, wr, -g.x * wi);   // Delta_i of the field after sweep t
+                acc = fma(dl, dl, acc);
+            }
+            bool sk = false;
+            const double2 gn = site_update<W1>(g, wr, wi, k2, sk);
+            if (commit) {
+                __stcs(dst + (size_t)i * 32 + lane, gn);
+                if (PAR == 1) {
+                    const double dl = fma(gn.y, wr, -gn.x * wi);   // Delta_i = Im(g_i conj w_i) after the update
+                    acc = fma(dl, dl, acc);
+                }
+                skipped |= sk;
+            }
+        }
+    }
+    return acc;
 }
 
 // Request the rows the NEXT site of this warp will read (its 2d neighbours and itself) into L1 while the current
@@ -296,24 +393,28 @@ __global__ void __launch_bounds__(kThreads, 1) relax_stream_kernel(const StreamP
             const bool commit = active && !fresh;
             const double2* E = rows(eb ^ 1);   // the values written by the last even half-sweep
             accO = 0.0;
-            for (int r = warp; r < half; r += kWarps) {
-                int i, jf[DIM], jb[DIM];
-                if (IDX::kPrefetch && kPrefetchAhead > 0 && r + kPrefetchAhead * kWarps < half) {
-                    IDX::locate(D, 1, r + kPrefetchAhead * kWarps, i, jf, jb);
-                    prefetch_rows<DIM>(E, A0, i, jf, jb, lane);
-                }
-                IDX::locate(D, 1, r, i, jf, jb);
-                double wr, wi;
-                neighbour_sum<DIM>(D, E, i, jf, jb, lane, wr, wi);
-                double2* own = A0 + (size_t)i * 32 + lane;
-                bool sk = false;
-                // own rows are read and written once per half-sweep: streaming hints keep L1 for the neighbour rows
-                const double2 gn = site_update<W1>(__ldcs(own), wr, wi, P.k2, sk);
-                if (commit) {
-                    __stcs(own, gn);
-                    const double dl = fma(gn.y, wr, -gn.x * wi);   // Delta_i = Im(g_i conj w_i) after the update
-                    accO = fma(dl, dl, accO);
-                    skipped |= sk;
+            if constexpr (IDX::kBlocksN > 0) {
+                accO = half_sweep_blocks<DIM, IDX::kBlocksN, 1, W1>(D, A0, A0, E, warp, lane, P.k2, commit, skipped);
+            } else {
+                for (int r = warp; r < half; r += kWarps) {
+                    int i, jf[DIM], jb[DIM];
+                    if (IDX::kPrefetch && kPrefetchAhead > 0 && r + kPrefetchAhead * kWarps < half) {
+                        IDX::locate(D, 1, r + kPrefetchAhead * kWarps, i, jf, jb);
+                        prefetch_rows<DIM>(E, A0, i, jf, jb, lane);
+                    }
+                    IDX::locate(D, 1, r, i, jf, jb);
+                    double wr, wi;
+                    neighbour_sum<DIM>(D, E, i, jf, jb, lane, wr, wi);
+                    double2* own = A0 + (size_t)i * 32 + lane;
+                    bool sk = false;
+                    // own rows are read and written once per half-sweep: streaming hints keep L1 for the neighbour rows
+                    const double2 gn = site_update<W1>(__ldcs(own), wr, wi, P.k2, sk);
+                    if (commit) {
+                        __stcs(own, gn);
+                        const double dl = fma(gn.y, wr, -gn.x * wi);   // Delta_i = Im(g_i conj w_i) after the update
+                        accO = fma(dl, dl, accO);
+                        skipped |= sk;
+                    }
                 }
             }
             if (commit) ++t;
@@ -327,23 +428,27 @@ __global__ void __launch_bounds__(kThreads, 1) relax_stream_kernel(const StreamP
         {
             const double2* E = rows(eb);
             double2* En = rows(eb ^ 1);
-            for (int r = warp; r < half; r += kWarps) {
-                int i, jf[DIM], jb[DIM];
-                if (IDX::kPrefetch && kPrefetchAhead > 0 && r + kPrefetchAhead * kWarps < half) {
-                    IDX::locate(D, 0, r + kPrefetchAhead * kWarps, i, jf, jb);
-                    prefetch_rows<DIM>(A0, E, i, jf, jb, lane);
-                }
-                IDX::locate(D, 0, r, i, jf, jb);
-                double wr, wi;
-                neighbour_sum<DIM>(D, A0, i, jf, jb, lane, wr, wi);
-                const double2 g = __ldcs(E + (size_t)i * 32 + lane);
-                const double dl = fma(g.y, wr, -g.x * wi);   // Delta_i of the field after sweep t
-                accE = fma(dl, dl, accE);
-                bool sk = false;
-                const double2 gn = site_update<W1>(g, wr, wi, P.k2, sk);
-                if (active) {
-                    __stcs(En + (size_t)i * 32 + lane, gn);
-                    skipped |= sk;
+            if constexpr (IDX::kBlocksN > 0) {
+                accE = half_sweep_blocks<DIM, IDX::kBlocksN, 0, W1>(D, E, En, A0, warp, lane, P.k2, active, skipped);
+            } else {
+                for (int r = warp; r < half; r += kWarps) {
+                    int i, jf[DIM], jb[DIM];
+                    if (IDX::kPrefetch && kPrefetchAhead > 0 && r + kPrefetchAhead * kWarps < half) {
+                        IDX::locate(D, 0, r + kPrefetchAhead * kWarps, i, jf, jb);
+                        prefetch_rows<DIM>(A0, E, i, jf, jb, lane);
+                    }
+                    IDX::locate(D, 0, r, i, jf, jb);
+                    double wr, wi;
+                    neighbour_sum<DIM>(D, A0, i, jf, jb, lane, wr, wi);
+                    const double2 g = __ldcs(E + (size_t)i * 32 + lane);
+                    const double dl = fma(g.y, wr, -g.x * wi);   // Delta_i of the field after sweep t
+                    accE = fma(dl, dl, accE);
+                    bool sk = false;
+                    const double2 gn = site_update<W1>(g, wr, wi, P.k2, sk);
+                    if (active) {
+                        __stcs(En + (size_t)i * 32 + lane, gn);
+                        skipped |= sk;
+                    }
                 }
             }
         }
