@@ -146,6 +146,27 @@ int u1gf_count_copies_host(uint64_t n, const double* F_norm_host, const double* 
                            int64_t* hist_host, int32_t nbins);
 
 /* ---------------------------------------------------------------------------------------------------------
+ * Read-outs of the sorted samples.
+ *
+ * u1gf_discovery_curve: the paper plots the number of distinct minima found as a function of the number of samples
+ * (Figs. 1-3).  With the copies numbered in order of first discovery (u1gf_count_copies),
+ *   curve[k] = number of copies c < n_distinct whose leader position rep[c] is < 2^k,   k = 0 .. n_levels-1
+ * i.e. the number of distinct copies among the first 2^k samples.  rep dev [n_distinct] int64 (as written by
+ * u1gf_count_copies), curve dev [n_levels] int64, 1 <= n_levels <= 65.
+ *
+ * u1gf_paper_count: the paper's own count: the number of distinct integers
+ * X = floor((1 - F_norm) * scale), scale = 1e8 in the paper, among the records with status bit0 clear.  It is
+ * reported beside n_distinct of u1gf_count_copies (R7: such keys can merge distinct copies and split a copy that
+ * straddles a key boundary).  F_norm dev [n], status dev [n], n_keys dev [1] int64, workspace dev scratch >=
+ * u1gf_paper_count_workspace_bytes(n), 256-byte aligned.
+ * Both calls are asynchronous on the stream, allocate nothing, and return U1GF_EINVAL on bad arguments.
+ * ------------------------------------------------------------------------------------------------------- */
+int u1gf_discovery_curve(uint64_t n_distinct, const int64_t* rep, int32_t n_levels, int64_t* curve, void* cuda_stream);
+size_t u1gf_paper_count_workspace_bytes(uint64_t n);
+int u1gf_paper_count(uint64_t n, const double* F_norm, const uint8_t* status, double scale, int64_t* n_keys,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------------------
  * Measurement helpers (not part of the method): roofline denominators measured on the device in use.
  *   u1gf_measure_fp64_peak   runs a dependent-chain-free DFMA kernel on all SMs for about `ms` milliseconds and
  *                            returns FP64 FMA instructions (thread-level) per second in *dfma_per_s.

@@ -268,3 +268,21 @@ def count_copies(F_norm, sig, status, tol_F=1e-10, tol_sig=1e-4, nbins=0, g_cano
         np.add.at(hist, b, multiplicity)
     return dict(copy_id=copy_id, n_distinct=n_distinct, rep=leaders, multiplicity=multiplicity, hist=hist,
                 F_rep=F[leaders], margins=margins)
+
+
+def discovery_curve(rep, n_levels):
+    """SURVEY 8(f)-1, PAPER.md:L149 / Figs. 1-3: curve[k] = number of copies whose first discovery (leader position,
+    `rep` as returned by count_copies) lies among the first 2^k samples, written out as the definition."""
+    rep = [int(r) for r in np.asarray(rep).ravel()]
+    return np.array([sum(1 for r in rep if r < (1 << k)) for k in range(int(n_levels))], dtype=np.int64)
+
+
+def paper_count(F_norm, status, scale=1e8):
+    """the paper converts x = 1 - F/(dV) into the integer X = floor(x * 1e8) and counts the
+    distinct integers among its converged samples."""
+    keys = set()
+    for f, st in zip(np.asarray(F_norm, dtype=np.float64).ravel(), np.asarray(status, dtype=np.uint8).ravel()):
+        if (int(st) & 1) == 0:
+            keys.add(int(np.floor((1.0 - float(f)) * float(scale))))
+    return len(keys)
+

@@ -36,6 +36,9 @@ _SIGNATURES = {
                                     _p, C.c_size_t, _p]),
     "u1gf_count_copies_host": (C.c_int, [C.c_uint64, _p, _p, _p, C.c_double, C.c_double, _p, _p, _p, _p, _p,
                                          C.c_int32]),
+    "u1gf_discovery_curve": (C.c_int, [C.c_uint64, _p, C.c_int32, _p, _p]),
+    "u1gf_paper_count_workspace_bytes": (C.c_size_t, [C.c_uint64]),
+    "u1gf_paper_count": (C.c_int, [C.c_uint64, _p, _p, C.c_double, _p, _p, C.c_size_t, _p]),
     "u1gf_measure_fp64_peak": (C.c_int, [C.c_double, C.POINTER(C.c_double), _p]),
     "u1gf_measure_fp64_rate": (C.c_int, [C.c_int32, C.c_double, C.POINTER(C.c_double), _p]),
     "u1gf_measure_smem_peak": (C.c_int, [C.c_double, C.POINTER(C.c_double), _p]),
@@ -235,6 +238,27 @@ def count_copies_host(F_norm, sig, status, tol_F=1e-10, tol_sig=1e-4, nbins=0):
                                         int(nbins)))
     k = int(nd[0])
     return dict(copy_id=copy_id, n_distinct=k, rep=rep[:k], multiplicity=mult[:k], hist=hist)
+
+
+def discovery_curve(rep, n_distinct: int, n_levels: int):
+    """u1gf_discovery_curve: rep = device int64 tensor from count_copies -> device int64 tensor [n_levels]."""
+    import torch
+    curve = torch.empty(int(n_levels), dtype=torch.int64, device="cuda")
+    _check(lib().u1gf_discovery_curve(int(n_distinct), _dev_ptr(rep), int(n_levels), _dev_ptr(curve), _stream()))
+    return curve
+
+
+def paper_count(F_norm, status, scale=1e8, workspace=None):
+    """u1gf_paper_count on device tensors -> device int64 tensor [1]."""
+    import torch
+    n = int(F_norm.numel())
+    nk = torch.zeros(1, dtype=torch.int64, device="cuda")
+    need = lib().u1gf_paper_count_workspace_bytes(n)
+    if workspace is None or workspace.numel() < need + 256:
+        workspace = _workspace(need)
+    _check(lib().u1gf_paper_count(n, _dev_ptr(F_norm), _dev_ptr(status), float(scale), _dev_ptr(nk),
+                                  _aligned_ptr(workspace), need, _stream()))
+    return nk
 
 
 def measure_fp64_peak(ms=200.0) -> float:

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libu1gf.so")
-SOURCES = ["orbit.cu", "relax_generic.cu", "relax_lanes.cu", "relax_stream.cu", "count_copies.cu", "check_fp.cu", "peaks.cu"]
+SOURCES = ["orbit.cu", "relax_generic.cu", "relax_lanes.cu", "relax_stream.cu", "count_copies.cu", "discovery.cu", "check_fp.cu", "peaks.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 

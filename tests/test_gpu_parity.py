@@ -313,3 +313,31 @@ def test_full_size_configs_sampled(b, oracle, cfg, orbit_idx, n_sample):
     gpu_ids = cid[ids]
     pairs = set(zip(gpu_ids.tolist(), oc["copy_id"].tolist()))
     assert len(pairs) == len(set(gpu_ids.tolist())) == len(set(oc["copy_id"].tolist()))
+
+
+@pytest.mark.gpu
+def test_discovery_curve_and_paper_count_match_oracle(b, oracle):
+    """SURVEY 8(f)-1 through the C-ABI: integer outputs, bit-exact against the oracle on the same device-produced
+    F / rep arrays (hot 4^3: hundreds of copies; 4x4: few copies; an empty batch)."""
+    import torch
+    for ext, seed, n in (((4, 4, 4), 3, 20000), ((4, 4), 1, 4096)):
+        orbit = b.Orbit(ext, synth.uniform_links(ext, seed))
+        r = b.relax_batch(orbit, seed, n)
+        c = b.count_copies(r["F_norm"], r["sig"], r["status"])
+        nd = int(c["n_distinct"].item())
+        rep = _cpu(c["rep"])[:nd]
+        for levels in (1, 16, 65):
+            cur = _cpu(b.discovery_curve(c["rep"], nd, levels))
+            assert (cur == oracle.discovery_curve(rep, levels)).all()
+        assert cur[-1] == nd
+        F, st = _cpu(r["F_norm"]), _cpu(r["status"])
+        for scale in (1e8, 1e4):
+            assert int(b.paper_count(r["F_norm"], r["status"], scale).item()) == oracle.paper_count(F, st, scale)
+        st2 = r["status"].clone()
+        st2[::3] |= 1                                    # not-converged records are ignored
+        assert int(b.paper_count(r["F_norm"], st2).item()) == oracle.paper_count(F, _cpu(st2))
+    e = torch.zeros(0, dtype=torch.float64, device="cuda")
+    assert int(b.paper_count(e, torch.zeros(0, dtype=torch.uint8, device="cuda")).item()) == 0
+    assert _cpu(b.discovery_curve(torch.zeros(1, dtype=torch.int64, device="cuda"), 0, 4)).tolist() == [0, 0, 0, 0]
+    with pytest.raises(b.U1gfError):
+        b.discovery_curve(torch.zeros(1, dtype=torch.int64, device="cuda"), 1, 66)

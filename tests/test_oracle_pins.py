@@ -498,3 +498,34 @@ def test_count_copies_hand_made_records(oracle):
     assert c2["copy_id"].tolist() == [0, 0, 0, 1]
     c0 = oracle.count_copies(np.zeros(0), np.zeros((0, 4)), np.zeros(0, np.uint8), nbins=4)
     assert c0["n_distinct"] == 0 and c0["hist"].tolist() == [0, 0, 0, 0]
+
+
+def test_discovery_curve_and_paper_count_pins(oracle):
+    """SURVEY 8(f)-1.  Discovery curve (Figs. 1-3) and the paper's floor(x*1e8) count (L133-135) on
+    records whose answers are known by construction, plus the properties that hold for any input."""
+    # copies first seen at positions 0, 1, 2, 5, 8, 1000: among the first 1, 2, 4, 8, 16, ... samples
+    rep = np.array([0, 1, 2, 5, 8, 1000])
+    assert oracle.discovery_curve(rep, 12).tolist() == [1, 2, 3, 4, 5, 5, 5, 5, 5, 5, 6, 6]
+    assert oracle.discovery_curve(np.zeros(0, np.int64), 3).tolist() == [0, 0, 0]
+    # ties to count_copies: the curve ends at n_distinct, never decreases, and curve[k] <= 2^k
+    F = np.array([0.50, 0.70, 0.50 + 2e-11, 0.61, 0.70 + 5e-11, 0.9, 0.33, 0.70])
+    sig = np.tile(np.array([.1, .2, .3, .4]), (8, 1))
+    c = oracle.count_copies(F, sig, np.zeros(8, np.uint8))
+    cur = oracle.discovery_curve(c["rep"], 5)           # copies first seen at positions 0, 1, 3, 5, 6
+    assert c["rep"].tolist() == [0, 1, 3, 5, 6]
+    assert cur.tolist() == [1, 2, 3, 5, 5] and cur[-1] == c["n_distinct"]
+    assert (np.diff(cur) >= 0).all() and all(cur[k] <= (1 << k) for k in range(5))
+    # paper count: x = 1 - F in units of 1e-8.  0.123456782 and 0.123456787 share the key 12345678; 0.123456793
+    # has the next key; a non-converged record is ignored; 1 - F is formed first, as the paper defines x
+    x = np.array([0.123456782, 0.123456787, 0.123456793, 0.5, 0.9])
+    st = np.array([0, 0, 0, 0, 1], dtype=np.uint8)
+    assert oracle.paper_count(1.0 - x, st) == 3
+    assert oracle.paper_count(1.0 - x, np.zeros(5, np.uint8)) == 4
+    assert oracle.paper_count(np.zeros(0), np.zeros(0, np.uint8)) == 0
+    # a coarser resolution merges: at 1e-2 the keys are 12, 12, 12, 50
+    assert oracle.paper_count(1.0 - x, st, scale=1e2) == 2
+    # R7 in one picture: two copies 3e-9 apart in F/(dV) that the signature separates are ONE key for the paper
+    Fc = np.array([0.6000000012, 0.6000000042])
+    sg = np.array([[.1, .2, .3, .4], [-.3, .2, .1, 0.]])
+    assert oracle.count_copies(Fc, sg, np.zeros(2, np.uint8))["n_distinct"] == 2
+    assert oracle.paper_count(Fc, np.zeros(2, np.uint8)) == 1
