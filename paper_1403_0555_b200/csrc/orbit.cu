@@ -186,6 +186,7 @@ int u1gf_create_orbit(int d, const int32_t* extents, const double* theta_host, u
     if (bL) {
         lanes_fill_links(d, D.ext, o->U_host.data(), (double2*)(h + off));
         o->U_lanes = (const double2*)(dptr + off);
+        o->U_lanes_host.assign((const double2*)(h + off), (const double2*)(h + off) + (size_t)V * d);
     }
     e = cudaMemcpy(o->blob, h, o->blob_bytes, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {

@@ -109,6 +109,7 @@ struct u1gf_orbit {
     int kernel_choice = 0;  // 0 auto, 1 generic, 2 streamed (falls back to generic where it does not apply)
     // device copy of the links in the layout of the specialised resident kernels (inside blob), or null
     const double2* U_lanes = nullptr;
+    std::vector<double2> U_lanes_host;  // host copy of the links part of that table (kernel parameter of the NB == 1 kernels)
 };
 
 namespace u1gf {
