@@ -87,8 +87,10 @@ def test_relax_gaussian_orbits_and_omega(b, oracle):
         orbit = b.Orbit(ext, th)
         for omega in (1.0, 1.7, 1.95):
             o = oracle.relax(ext, th, seed, n, omega=omega, want_g=True)
-            r = _gpu_relax(b, orbit, seed, n, omega=omega, want_g=True)
-            _compare_relax(o, r, orbit.V)
+            for kernel in (0, 2):                       # the resident kernel and the streamed one forced onto it
+                orbit.set_kernel(kernel)
+                r = _gpu_relax(b, orbit, seed, n, omega=omega, want_g=True)
+                _compare_relax(o, r, orbit.V)
 
 
 def test_relax_options(b, oracle):
@@ -96,7 +98,7 @@ def test_relax_options(b, oracle):
     ext = (4, 4, 4)
     th = synth.uniform_links(ext, 3)
     orbit = b.Orbit(ext, th)
-    for kernel in (0, 1):
+    for kernel in (0, 1, 2):                            # resident, generic, streamed
         orbit.set_kernel(kernel)
         ids = np.array([5, 3, 2 ** 40 + 7, 3, 2 ** 63 + 11, 0], dtype=np.uint64)
         seed = (9 << 32) | 1234567
@@ -123,7 +125,7 @@ def test_relax_is_deterministic_and_batch_independent(b):
     """A start's result is a pure function of (orbit, seed, index): identical bits whether it runs alone, in a big
     batch, through start_ids or twice (include/u1gf.h contract; the representative re-relaxation relies on it)."""
     import torch
-    for ext, seed in [((4, 4, 4, 4), 12), ((8, 8), 2), ((4, 4), 1), ((3, 3, 3, 3), 12)]:
+    for ext, seed in [((4, 4, 4, 4), 12), ((8, 8), 2), ((4, 4), 1), ((3, 3, 3, 3), 12), ((8, 8, 8), 21)]:
         orbit = b.Orbit(ext, synth.uniform_links(ext, seed))
         big = b.relax_batch(orbit, seed, 3000, want_g=False)
         again = b.relax_batch(orbit, seed, 3000)
