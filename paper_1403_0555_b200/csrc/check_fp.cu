@@ -71,18 +71,26 @@ __device__ __forceinline__ int sturm_count(const double* alpha, const double* be
     double p0 = 1.0, p1 = alpha[0] - x;
     if (p1 == 0.0) p1 = 1e-300;
     int cnt = p1 < 0.0 ? 1 : 0;
-    for (int j = 1; j < k; ++j) {
-        double p2 = fma(alpha[j] - x, p1, -beta2[j - 1] * p0);
+    auto step = [&](double d, double b2) {
+        double p2 = fma(d, p1, -b2 * p0);
         if (p2 == 0.0) p2 = p1 * 1e-300;   // a vanishing minor takes the sign of its predecessor: no change
         cnt += ((p2 < 0.0) != (p1 < 0.0)) ? 1 : 0;
         p0 = p1;
         p1 = p2;
-        if ((j & 7) == 7) {
-            const double sc = unit_scale(p1);
-            p0 *= sc;
-            p1 *= sc;
-        }
+    };
+    int j = 1;
+    for (; j + 3 < k; j += 4) {   // the shared-memory operands of four steps are fetched ahead of the dependent chain
+        const double d0 = alpha[j] - x, d1 = alpha[j + 1] - x, d2 = alpha[j + 2] - x, d3 = alpha[j + 3] - x;
+        const double b0 = beta2[j - 1], b1 = beta2[j], b2 = beta2[j + 1], b3 = beta2[j + 2];
+        step(d0, b0);
+        step(d1, b1);
+        step(d2, b2);
+        step(d3, b3);
+        const double sc = unit_scale(p1);   // |p| grows at most by (4 d + 1)^4 per round: far from overflow
+        p0 *= sc;
+        p1 *= sc;
     }
+    for (; j < k; ++j) step(alpha[j] - x, beta2[j - 1]);
     return cnt;
 }
 
@@ -101,7 +109,7 @@ __device__ double smallest_ritz(const double* alpha, const double* beta2, int k,
             hi = lo + h * (double)(f + 1);
             lo = lo + h * (double)f;
         }
-        if (hi - lo <= 4e-16 * fmax(1.0, fmax(fabs(lo), fabs(hi)))) break;
+        if (hi - lo <= 2e-14 * fmax(1.0, fmax(fabs(lo), fabs(hi)))) break;   // lambda_1 is compared at 1e-8 (R9, R16)
     }
     return 0.5 * (lo + hi);
 }
@@ -177,7 +185,9 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
         double* v1 = va;  // current Lanczos vector
         double* v0 = vb;  // previous one; overwritten by the new direction
         double beta_prev = 0.0, lam = 0.0, lam_hi = 4.0 * DIM + 1.0;
-        int k = 0, next_check = 8;
+        int k = 0, next_check = 16, k_prev = 0, n_checks = 0;
+        double res_prev = 0.0, last_drop = 0.0;
+        bool have_drop = false;
         bool done = false;
         while (!done) {
             // w = M v1 - beta_prev v0  (into v0), alpha = <w, v1>
@@ -223,7 +233,14 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
             if (breakdown || k == kmax || k == next_check) {
                 __syncthreads();
                 if (tid < 32) {
-                    const double l = smallest_ritz(alpha, beta2, k, -(4.0 * DIM + 1.0), lam_hi);
+                    // Ritz values decrease with k (interlacing): the new one lies below the last; a lower end a few
+                    // times the last decrease below it is tried first (one Sturm count says whether it holds)
+                    double lo_try = -(4.0 * DIM + 1.0);
+                    if (have_drop) {
+                        const double cand = lam - 8.0 * last_drop - 1e-9;
+                        if (sturm_count(alpha, beta2, k, cand) == 0) lo_try = cand;
+                    }
+                    const double l = smallest_ritz(alpha, beta2, k, lo_try, lam_hi);
                     const double res = breakdown ? 0.0 : b * last_component(alpha, beta, ibeta, k, l - 1e-13);
                     if (tid == 0) {
                         s_lam = l;
@@ -231,10 +248,24 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
                     }
                 }
                 __syncthreads();
+                if (n_checks > 0) {
+                    last_drop = fmax(lam - s_lam, 0.0);
+                    have_drop = true;
+                }
                 lam = s_lam;
-                lam_hi = lam + 1e-9;  // Ritz values decrease with k (interlacing)
-                if (breakdown || k == kmax || s_res < 1e-10) done = true;
-                next_check = k + max(4, k / 4);
+                lam_hi = lam + 1e-9;
+                const double res = s_res;
+                if (breakdown || k == kmax || res < 1e-10) done = true;
+                // next test where the residual bound, which falls geometrically, is expected to cross 1e-10
+                int step = max(4, k / 4);
+                if (n_checks > 0 && res > 0.0 && res < res_prev) {
+                    const double per_step = log(res_prev / res) / (double)(k - k_prev);
+                    step = max(3, min(step, (int)(0.9 * log(res / 1e-10) / per_step) + 1));
+                }
+                res_prev = res;
+                k_prev = k;
+                ++n_checks;
+                next_check = k + step;
             }
             if (!done) {
                 const double ib = 1.0 / b;
