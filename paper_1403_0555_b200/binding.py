@@ -163,16 +163,35 @@ def relax_batch(orbit: Orbit, seed, n_starts, *, first_start=0, start_ids=None, 
     return out
 
 
+def host_buffers(n, V=0, want_g=False, pinned=True):
+    """Result arrays for the *_host calls (F_norm, sweeps, status, sig, copy_id, rep, multiplicity[, g_canon]) in
+    page-locked host memory (numpy views of pinned torch tensors), so that the library's device<->host copies run at
+    PCIe speed and a caller can reuse them across calls instead of faulting in fresh pages every time."""
+    import torch
+
+    def arr(shape, dtype):
+        return torch.empty(shape, dtype=dtype, pin_memory=pinned).numpy()
+    n = int(n)
+    return dict(F_norm=arr(n, torch.float64), sweeps=arr(n, torch.int32), status=arr(n, torch.uint8),
+                sig=arr((n, 4), torch.float64), copy_id=arr(n, torch.int32), rep=arr(max(n, 1), torch.int64),
+                multiplicity=arr(max(n, 1), torch.int64),
+                g_canon=arr((n, int(V), 2), torch.float64) if want_g else None)
+
+
 def relax_batch_host(orbit: Orbit, seed, n_starts, *, first_start=0, start_ids=None, omega=1.7, eps=1e-13,
-                     max_sweeps=20000, check_every=1, want_g=False):
-    """u1gf_relax_batch_host: numpy result arrays, device<->host copies inside the call."""
+                     max_sweeps=20000, check_every=1, want_g=False, out=None):
+    """u1gf_relax_batch_host: numpy result arrays, device<->host copies inside the call.  `out` (host_buffers())
+    supplies the result arrays; otherwise fresh pageable ones are made."""
     ids = None
     if start_ids is not None:
         ids = np.ascontiguousarray(start_ids, dtype=np.uint64)
         n_starts = ids.size
     n = int(n_starts)
-    out = dict(F_norm=np.zeros(n), sweeps=np.zeros(n, dtype=np.int32), status=np.zeros(n, dtype=np.uint8),
-               sig=np.zeros((n, 4)), g_canon=np.zeros((n, orbit.V, 2)) if want_g else None)
+    if out is None:
+        out = dict(F_norm=np.zeros(n), sweeps=np.zeros(n, dtype=np.int32), status=np.zeros(n, dtype=np.uint8),
+                   sig=np.zeros((n, 4)), g_canon=np.zeros((n, orbit.V, 2)) if want_g else None)
+    elif out["F_norm"].size != n or (want_g and out.get("g_canon") is None):
+        raise ValueError("relax_batch_host: `out` buffers do not match n_starts / want_g")
     _check(lib().u1gf_relax_batch_host(orbit.handle, int(seed), int(first_start), n, _np_ptr(ids), float(omega),
                                        float(eps), int(max_sweeps), int(check_every), _np_ptr(out["F_norm"]),
                                        _np_ptr(out["sweeps"]), _np_ptr(out["status"]), _np_ptr(out["sig"]),
@@ -223,15 +242,18 @@ def count_copies(F_norm, sig, status, tol_F=1e-10, tol_sig=1e-4, nbins=0, worksp
     return dict(copy_id=copy_id, n_distinct=nd, rep=rep, multiplicity=mult, hist=hist, workspace=workspace)
 
 
-def count_copies_host(F_norm, sig, status, tol_F=1e-10, tol_sig=1e-4, nbins=0):
+def count_copies_host(F_norm, sig, status, tol_F=1e-10, tol_sig=1e-4, nbins=0, out=None):
     F = np.ascontiguousarray(F_norm, dtype=np.float64)
     S = np.ascontiguousarray(sig, dtype=np.float64).reshape(-1, 4)
     st = np.ascontiguousarray(status, dtype=np.uint8)
     n = F.size
-    copy_id = np.zeros(n, dtype=np.int32)
     nd = np.zeros(1, dtype=np.int64)
-    rep = np.zeros(max(n, 1), dtype=np.int64)
-    mult = np.zeros(max(n, 1), dtype=np.int64)
+    if out is not None and out["copy_id"].size == n:
+        copy_id, rep, mult = out["copy_id"], out["rep"], out["multiplicity"]
+    else:
+        copy_id = np.zeros(n, dtype=np.int32)
+        rep = np.zeros(max(n, 1), dtype=np.int64)
+        mult = np.zeros(max(n, 1), dtype=np.int64)
     hist = np.zeros(nbins, dtype=np.int64) if nbins else None
     _check(lib().u1gf_count_copies_host(n, _np_ptr(F), _np_ptr(S), _np_ptr(st), float(tol_F), float(tol_sig),
                                         _np_ptr(copy_id), _np_ptr(nd), _np_ptr(rep), _np_ptr(mult), _np_ptr(hist),
