@@ -173,8 +173,14 @@ int u1gf_paper_count(uint64_t n, const double* F_norm, const uint8_t* status, do
  *   u1gf_measure_fp64_rate   the same rate for a DFMA stream of a given operand pattern: 0 = the stream of
  *                            u1gf_measure_fp64_peak (one register operand, two constants); 1 = three distinct
  *                            register operands per DFMA; 2 = the complex multiply-accumulate pattern of the
- *                            neighbour sum w_i (Eq. 5).  Patterns 1 and 2 are limited by register-file
- *                            operand bandwidth, not by the FP64 lanes.
+ *                            neighbour sum w_i (Eq. 5); 3 / 4 = stream 0 / stream 1 with two independent
+ *                            integer instructions per DFMA (FP64 FMAs counted only); 5 = one dependent chain per
+ *                            warp, one warp per scheduler (rate = threads in flight / dependent-issue latency);
+ *                            6 = FP64 tensor-core DMMA m8n8k4, 8 FMAs per thread and instruction.  Patterns 1-4
+ *                            are limited by register-file operand bandwidth, not by the FP64 lanes.
+ *   u1gf_measure_smem_rate   warp-level shared-memory instructions per second of a mix: 0 = 4 lane-strided LDS.128
+ *                            + 1 STS.128 (neighbours of 32 starts and the store), 1 = 8 warp-uniform LDS.128
+ *                            (links), 2 = both (the 13 shared-memory instructions of one 4^4 site update).
  *   u1gf_measure_smem_peak   same for 128-bit conflict-free shared-memory loads, bytes per second.
  *   u1gf_last_launch_count   kernels launched by the calling thread's most recent compute call.
  *   u1gf_last_relax_ms       device time (CUDA events on the call's stream) of the relaxation kernel of the
@@ -184,6 +190,7 @@ int u1gf_paper_count(uint64_t n, const double* F_norm, const uint8_t* status, do
 int u1gf_measure_fp64_peak(double ms, double* dfma_per_s, void* cuda_stream);
 int u1gf_measure_fp64_rate(int32_t pattern, double ms, double* dfma_per_s, void* cuda_stream);
 int u1gf_measure_smem_peak(double ms, double* bytes_per_s, void* cuda_stream);
+int u1gf_measure_smem_rate(int32_t mix, double ms, double* instr_per_s, void* cuda_stream);
 int32_t u1gf_last_launch_count(void);
 double u1gf_last_relax_ms(void);
 

@@ -42,6 +42,7 @@ _SIGNATURES = {
     "u1gf_measure_fp64_peak": (C.c_int, [C.c_double, C.POINTER(C.c_double), _p]),
     "u1gf_measure_fp64_rate": (C.c_int, [C.c_int32, C.c_double, C.POINTER(C.c_double), _p]),
     "u1gf_measure_smem_peak": (C.c_int, [C.c_double, C.POINTER(C.c_double), _p]),
+    "u1gf_measure_smem_rate": (C.c_int, [C.c_int32, C.c_double, C.POINTER(C.c_double), _p]),
     "u1gf_last_launch_count": (C.c_int32, []),
     "u1gf_last_relax_ms": (C.c_double, []),
 }
@@ -298,6 +299,12 @@ def measure_fp64_rate(pattern: int, ms=200.0) -> float:
 def measure_smem_peak(ms=200.0) -> float:
     v = C.c_double(0)
     _check(lib().u1gf_measure_smem_peak(float(ms), C.byref(v), _stream()))
+    return v.value
+
+
+def measure_smem_rate(mix: int, ms=200.0) -> float:
+    v = C.c_double(0)
+    _check(lib().u1gf_measure_smem_rate(int(mix), float(ms), C.byref(v), _stream()))
     return v.value
 
 
