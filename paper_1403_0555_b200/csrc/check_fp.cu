@@ -145,10 +145,14 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
     double* va = c + (size_t)V * DIM;  // [V]
     double* vb = va + V;            // [V]
     __shared__ double red[2][32], red2[2][32];
-    __shared__ double alpha[kMaxK], beta[kMaxK], beta2[kMaxK], ibeta[kMaxK];
+    const int kcap = min(V - 1, kMaxK);
+    double* alpha = vb + V;   // Lanczos coefficients [4][kcap], behind the vectors in dynamic shared memory
+    double* beta = alpha + kcap;
+    double* beta2 = beta + kcap;
+    double* ibeta = beta2 + kcap;
     __shared__ double s_lam, s_res;
     int buf = 0;
-    const int kmax = min(V - 1, kMaxK);
+    const int kmax = kcap;
 
     for (unsigned long long cfg = blockIdx.x; cfg < P.n_cfg; cfg += gridDim.x) {
         const double2* g = P.g + cfg * (unsigned long long)V;
@@ -293,12 +297,19 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
 template <int DIM>
 int launch(const u1gf_orbit* o, const FpParams& P, cudaStream_t st) {
     const int V = o->dev.V;
-    const size_t smem = ((size_t)V * DIM + 2 * (size_t)V) * sizeof(double);
+    const int kcap = V - 1 < kMaxK ? V - 1 : kMaxK;
+    const size_t smem = ((size_t)V * DIM + 2 * (size_t)V + 4 * (size_t)(kcap > 0 ? kcap : 1)) * sizeof(double);
     if (smem > 220 * 1024)
         return fail(U1GF_EINVAL, "u1gf_check_fp: lattice of %d sites does not fit the resident Lanczos kernel", V);
     auto kern = lanczos_kernel<DIM>;
     if (smem > 48 * 1024) U1GF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int T = (V + 31) / 32 * 32;
+    // few threads per configuration: the Ritz test is serial work of one warp, during which the other warps of the
+    // CTA wait; many small CTAs per SM keep the SM busy with other configurations meanwhile (measured: 8 warps per
+    // configuration spent 54 % of their time at that barrier)
+#ifndef U1GF_FP_SITES_PER_THREAD
+#define U1GF_FP_SITES_PER_THREAD 8
+#endif
+    int T = ((V + U1GF_FP_SITES_PER_THREAD - 1) / U1GF_FP_SITES_PER_THREAD + 31) / 32 * 32;
     if (T > 512) T = 512;
     int per_sm = 0;
     U1GF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T, smem));
