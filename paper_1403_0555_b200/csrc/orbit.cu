@@ -220,7 +220,9 @@ static bool use_stream(const u1gf_orbit* o) {
 
 const char* u1gf_kernel_name(const u1gf_orbit* o) {
     if (!o) return "";
-    return use_lanes(o) ? lanes_name(o) : use_stream(o) ? "stream_lane_per_start" : "generic_cta_per_start";
+    return use_lanes(o)    ? lanes_name(o)
+           : use_stream(o) ? (o->dev.all_even ? "stream_lane_per_start" : "phased_lane_per_start")
+                           : "generic_cta_per_start";
 }
 
 size_t u1gf_relax_workspace_bytes(const u1gf_orbit* o, uint64_t n_starts) {

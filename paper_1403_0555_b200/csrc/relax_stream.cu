@@ -466,6 +466,192 @@ __global__ void __launch_bounds__(kThreads, 1) relax_stream_kernel(const StreamP
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Lattices with odd extents (3^4, 5x3x2, ...): the same lane-per-start layout, one small CTA (4 warps) per team, the
+// update phases of reading R3 (parity, then level) from the orbit's tables with a CTA barrier after each, and the
+// gauge precision from a separate pass over the post-sweep field (on an odd ring a same-parity neighbour may still
+// move after w_i was formed, so the fused measure of the even lattices is not exact here: R5).  A team's field
+// (V x 512 bytes: 41 KB at 3^4) stays in L1; four teams share an SM.
+// ---------------------------------------------------------------------------------------------------------
+constexpr int kPhasedThreads = 128;
+constexpr int kPhasedWarps = kPhasedThreads / 32;
+
+template <int DIM, bool W1>
+__global__ void __launch_bounds__(kPhasedThreads, 4) relax_phased_kernel(const StreamParams P) {
+    constexpr unsigned FULL = 0xffffffffu;
+    __shared__ double red[2][kPhasedWarps][5];
+    __shared__ double sred[2][kPhasedWarps][32];
+    __shared__ unsigned long long s_pos[32];
+    __shared__ unsigned s_skip[32];
+    __shared__ unsigned long long s_k;
+    const OrbitDev& D = P.D;
+    const int V = D.V;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double2* const A = P.team_buf + (size_t)blockIdx.x * V * 32;   // [V][32 starts]
+
+    bool active = false, maxed = false, skipped = false;
+    int t = 0, rb = 0, fb = 0;
+    unsigned need = FULL, dumpm = 0;
+
+    auto sum5 = [&](double (&v)[5]) {   // CTA sum, same result in every thread, fixed order
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+            for (int q = 0; q < 5; ++q) v[q] += __shfl_down_sync(FULL, v[q], o);
+        if (lane == 0)
+#pragma unroll
+            for (int q = 0; q < 5; ++q) red[fb][warp][q] = v[q];
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+            double sacc = 0.0;
+            for (int w = 0; w < kPhasedWarps; ++w) sacc += red[fb][w][q];
+            v[q] = sacc;
+        }
+        fb ^= 1;
+    };
+
+    for (;;) {
+        // ---------------------------------------------------------- service (CTA-uniform): finalise, refill
+        for (unsigned m = need; m; m &= m - 1) {
+            const int L = __ffs(m) - 1;
+            if ((dumpm >> L) & 1u) {   // a5, a6 for the start of lane L
+                if (skipped) atomicOr(&s_skip[lane], 1u);
+                const int tL = __shfl_sync(FULL, t, L);
+                const int mxL = __shfl_sync(FULL, maxed ? 1 : 0, L);
+                const unsigned long long k = s_pos[L];
+                const double2 c = A[(size_t)(V - 1) * 32 + L];
+                double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+                for (int i = tid; i < V; i += kPhasedThreads) {
+                    const double2 gi = A[(size_t)i * 32 + L];
+#pragma unroll
+                    for (int mu = 0; mu < DIM; ++mu) {   // F = sum Re(g_i U_{i,mu} conj g_{i+mu})   (Eq. 3)
+                        const double2 u = __ldg(D.U + i * DIM + mu);
+                        const double2 gj = A[(size_t)__ldg(D.fwd + i * DIM + mu) * 32 + L];
+                        const double ar = fma(gi.x, u.x, -gi.y * u.y), ai = fma(gi.x, u.y, gi.y * u.x);
+                        v[0] += fma(ar, gj.x, ai * gj.y);
+                    }
+                    const double re = fma(gi.x, c.x, gi.y * c.y);   // g~ = g conj(g_{V-1})
+                    const double im = fma(gi.y, c.x, -gi.x * c.y);
+                    const unsigned bits = __ldg(D.sgn + i);
+                    v[1] += ((bits & 1u) ? re : -re) + ((bits & 16u) ? im : -im);
+                    v[2] += ((bits & 2u) ? re : -re) + ((bits & 32u) ? im : -im);
+                    v[3] += ((bits & 4u) ? re : -re) + ((bits & 64u) ? im : -im);
+                    v[4] += ((bits & 8u) ? re : -re) + ((bits & 128u) ? im : -im);
+                    if (P.g_canon) reinterpret_cast<double2*>(P.g_canon)[k * (unsigned long long)V + i] = make_double2(re, im);
+                }
+                sum5(v);   // its barrier also publishes the s_skip bits
+                if (tid == 0) {
+                    P.F_norm[k] = v[0] / ((double)DIM * (double)V);
+                    P.sweeps[k] = tL;
+                    P.status[k] = (uint8_t)((mxL ? 1 : 0) | (s_skip[L] ? 2 : 0));
+                    reinterpret_cast<double4*>(P.sig)[k] =
+                        make_double4(v[1] / (double)V, v[2] / (double)V, v[3] / (double)V, v[4] / (double)V);
+                }
+            }
+            if (tid == 0) s_k = atomicAdd(P.counter, 1ull);
+            __syncthreads();
+            const unsigned long long k = s_k;
+            if (k < P.n_starts) {
+                const uint64_t s = P.start_ids ? P.start_ids[k] : P.first_start + k;
+                for (int i = tid; i < V; i += kPhasedThreads) {   // a2
+                    const u32x4 r = philox((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 0u, (uint32_t)P.seed,
+                                           (uint32_t)(P.seed >> 32));
+                    double sn, cs;
+                    sincospi(unit_interval_pm1(r.x, r.y), &sn, &cs);
+                    A[(size_t)i * 32 + L] = make_double2(cs, sn);
+                }
+                if (tid == 0) {
+                    s_pos[L] = k;
+                    s_skip[L] = 0u;
+                }
+                if (lane == L) {
+                    active = true;
+                    t = 0;
+                    skipped = false;
+                }
+            } else if (lane == L) {
+                active = false;
+            }
+            __syncthreads();
+        }
+        if (__ballot_sync(FULL, active) == 0) break;   // every warp holds the same lane states
+
+        // ---------------------------------------------------------- one sweep: the phases of R3, in place
+        for (int p = 0; p < D.n_phases; ++p) {
+            const int q1 = D.phase_off[p + 1];
+            for (int q = D.phase_off[p] + warp; q < q1; q += kPhasedWarps) {
+                int i, jf[DIM], jb[DIM];
+                i = __ldg(D.order + q);
+#pragma unroll
+                for (int mu = 0; mu < DIM; ++mu) {
+                    jf[mu] = __ldg(D.fwd + i * DIM + mu);
+                    jb[mu] = __ldg(D.bwd + i * DIM + mu);
+                }
+                double wr, wi;
+                neighbour_sum<DIM>(D, A, i, jf, jb, lane, wr, wi);
+                double2* own = A + (size_t)i * 32 + lane;
+                bool sk = false;
+                const double2 gn = site_update<W1>(*own, wr, wi, P.k2, sk);
+                if (active) {
+                    *own = gn;
+                    skipped |= sk;
+                }
+            }
+            __syncthreads();
+        }
+        if (active) ++t;
+
+        // ---------------------------------------------------------- a4: gauge precision of the post-sweep field
+        double acc = 0.0;
+        for (int i = warp; i < V; i += kPhasedWarps) {
+            int jf[DIM], jb[DIM];
+#pragma unroll
+            for (int mu = 0; mu < DIM; ++mu) {
+                jf[mu] = __ldg(D.fwd + i * DIM + mu);
+                jb[mu] = __ldg(D.bwd + i * DIM + mu);
+            }
+            double wr, wi;
+            neighbour_sum<DIM>(D, A, i, jf, jb, lane, wr, wi);
+            const double2 g = A[(size_t)i * 32 + lane];
+            const double dl = fma(g.y, wr, -g.x * wi);   // Delta_i = Im(g_i conj w_i)
+            acc = fma(dl, dl, acc);
+        }
+        sred[rb][warp][lane] = acc;
+        __syncthreads();
+        double S = 0.0;
+#pragma unroll
+        for (int w = 0; w < kPhasedWarps; ++w) S += sred[rb][w][lane];
+        rb ^= 1;
+        const bool conv = active && (t % P.check_every == 0) && (S / (double)V < P.eps);
+        maxed = active && !conv && t == P.max_sweeps;
+        dumpm = __ballot_sync(FULL, conv || maxed);
+        need = dumpm;
+    }
+}
+
+template <int DIM, bool W1>
+int launch_phased_k(const u1gf_orbit* o, const RelaxArgs& a, StreamParams& P, cudaStream_t st) {
+    auto kern = relax_phased_kernel<DIM, W1>;
+    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 5);
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kPhasedThreads, 0) != cudaSuccess) per_sm = 0;
+    unsigned long long teams = (unsigned long long)per_sm * (unsigned long long)o->sm_count;
+    const unsigned long long batches = (a.n_starts + 31) / 32;
+    if (teams > batches) teams = batches;
+    if (teams > 4ull * (unsigned long long)o->sm_count) teams = 4ull * (unsigned long long)o->sm_count;   // workspace bound
+    if (teams < 1) return fail(U1GF_ECUDA, "phased relaxation kernel does not fit on an SM");
+    const size_t bytes = 256 + (size_t)teams * (size_t)o->dev.V * 32 * sizeof(double2);
+    U1GF_CUDA(cudaMemsetAsync(a.workspace, 0, bytes, st));
+    U1GF_CUDA(cudaEventRecord(t_ev0, st));
+    kern<<<(unsigned)teams, kPhasedThreads, 0, st>>>(P);
+    U1GF_CUDA(cudaGetLastError());
+    U1GF_CUDA(cudaEventRecord(t_ev1, st));
+    t_ev_valid = true;
+    ++t_launches;
+    return U1GF_OK;
+}
+
 template <int DIM, bool W1, class IDX>
 int launch_k(const u1gf_orbit* o, const RelaxArgs& a, StreamParams& P, cudaStream_t st) {
     auto kern = relax_stream_kernel<DIM, W1, IDX>;
@@ -511,7 +697,22 @@ bool cubic(const u1gf_orbit* o, int n) {
 }
 
 template <int DIM>
+int launch_phased(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st) {
+    const bool w1 = a.omega == 1.0;
+    StreamParams P;
+    P.seed = a.seed; P.first_start = a.first_start; P.n_starts = a.n_starts; P.start_ids = a.start_ids;
+    P.k2 = w1 ? 0.0 : a.omega / (1.0 - a.omega); P.eps = a.eps;
+    P.max_sweeps = a.max_sweeps; P.check_every = a.check_every;
+    P.F_norm = a.F_norm; P.sweeps = a.sweeps; P.status = a.status; P.sig = a.sig; P.g_canon = a.g_canon;
+    P.counter = (unsigned long long*)a.workspace;
+    P.team_buf = (double2*)((char*)a.workspace + 256);
+    P.D = o->dev;
+    return w1 ? launch_phased_k<DIM, true>(o, a, P, st) : launch_phased_k<DIM, false>(o, a, P, st);
+}
+
+template <int DIM>
 int launch(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st) {
+    if (!o->dev.all_even) return launch_phased<DIM>(o, a, st);
     if (DIM >= 2) {
         if (cubic<DIM>(o, 6)) return launch_w<DIM, Cubic<DIM, 6>>(o, a, st);
         if (cubic<DIM>(o, 8)) return launch_w<DIM, Cubic<DIM, 8>>(o, a, st);
@@ -524,11 +725,16 @@ int launch(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st) {
 
 // every extent even (two-colour checkerboard); chosen automatically from 512 sites up, where a team's field no longer
 // fits on chip and the generic kernel's per-start link traffic dominates
-bool stream_supported(const u1gf_orbit* o) { return o->dev.all_even && o->dev.d >= 1 && o->dev.d <= 4; }
-bool stream_preferred(const u1gf_orbit* o) { return stream_supported(o) && o->dev.V >= 512; }
+bool stream_supported(const u1gf_orbit* o) { return o->dev.d >= 1 && o->dev.d <= 4; }
+// automatic choice: all-even lattices from 512 sites up (the fused two-colour kernel), lattices with an odd extent from
+// 64 sites up (the phased kernel; 3^4 = 81)
+bool stream_preferred(const u1gf_orbit* o) {
+    return stream_supported(o) && (o->dev.all_even ? o->dev.V >= 512 : o->dev.V >= 64);
+}
 
 size_t stream_workspace_bytes(const u1gf_orbit* o, uint64_t n) {
-    // upper bound on the teams of a launch: 2 CTAs per SM, never more than the batches of 32 starts
+    // upper bound on the teams of a launch: 2 CTAs per SM with two buffers each (even lattices) or 4 CTAs per SM with
+    // one buffer (odd extents): the same bytes; never more than the batches of 32 starts
     unsigned long long teams = 2ull * (unsigned long long)o->sm_count;
     const unsigned long long batches = (n + 31) / 32;
     if (teams > batches) teams = batches;

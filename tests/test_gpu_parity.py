@@ -64,13 +64,13 @@ def test_relax_matches_oracle(b, oracle, ext, seed, n, kernel):
     orbit.set_kernel(kernel)
     if kernel == 1 and orbit.kernel_name != "generic_cta_per_start":
         pytest.fail("set_kernel(1) must select the generic kernel")
-    if kernel == 2:
-        if any(e % 2 for e in ext):
-            pytest.skip("the streamed kernel needs even extents")
-        if orbit.kernel_name != "stream_lane_per_start":
-            pytest.fail("set_kernel(2) must select the streamed kernel on an all-even lattice")
-    if kernel == 0 and orbit.V >= 512 and not any(e % 2 for e in ext):
+    odd = any(e % 2 for e in ext)
+    if kernel == 2 and orbit.kernel_name != ("phased_lane_per_start" if odd else "stream_lane_per_start"):
+        pytest.fail("set_kernel(2) must select the streamed (all-even) / phased (odd extent) lane-per-start kernel")
+    if kernel == 0 and orbit.V >= 512 and not odd:
         assert orbit.kernel_name == "stream_lane_per_start"
+    if kernel == 0 and orbit.V >= 64 and odd:
+        assert orbit.kernel_name == "phased_lane_per_start"
     V = orbit.V
     eps = 1e-12 if V > 256 else 1e-13
     o = oracle.relax(ext, th, seed, n, eps=eps, want_g=True)
