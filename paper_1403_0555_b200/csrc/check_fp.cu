@@ -35,28 +35,6 @@ __device__ __forceinline__ double block_sum(double a, double (*red)[32], int& bu
     return s;
 }
 
-__device__ __forceinline__ void block_sum2(double& a, double& b, double (*red)[32], double (*red2)[32], int& buf) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        a += __shfl_down_sync(0xffffffffu, a, o);
-        b += __shfl_down_sync(0xffffffffu, b, o);
-    }
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
-    if (lane == 0) {
-        red[buf][warp] = a;
-        red2[buf][warp] = b;
-    }
-    __syncthreads();
-    double sa = 0.0, sb = 0.0;
-    for (int w = 0; w < nw; ++w) {
-        sa += red[buf][w];
-        sb += red2[buf][w];
-    }
-    a = sa;
-    b = sb;
-    buf ^= 1;
-}
-
 // power of two that brings |p| back near 1 (0 and denormals: no scaling)
 __device__ __forceinline__ double unit_scale(double p) {
     const int e = (__double2hiint(p) >> 20) & 0x7ff;
@@ -144,7 +122,7 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
     double* c = sm;                 // [V*DIM]
     double* va = c + (size_t)V * DIM;  // [V]
     double* vb = va + V;            // [V]
-    __shared__ double red[2][32], red2[2][32];
+    __shared__ double red[2][32];
     const int kcap = min(V - 1, kMaxK);
     double* alpha = vb + V;   // Lanczos coefficients [4][kcap], behind the vectors in dynamic shared memory
     double* beta = alpha + kcap;

@@ -21,10 +21,6 @@ namespace {
 
 constexpr int kThreads = 512;
 constexpr int kWarps = kThreads / 32;
-#ifndef U1GF_STREAM_AHEAD
-#define U1GF_STREAM_AHEAD 0
-#endif
-constexpr int kPrefetchAhead = U1GF_STREAM_AHEAD;   // sites of this warp between a prefetch and its use
 
 struct StreamParams {
     uint64_t seed, first_start, n_starts;
@@ -108,13 +104,12 @@ __device__ __forceinline__ int parity_of(const OrbitDev& D, int i) {
     return p & 1;
 }
 
-// Where the r-th site of parity p sits and who its neighbours are.  Tables: the orbit's order / fwd / bwd arrays (any
-// all-even lattice; three dependent global loads before the first row can be requested).  Cubic<N>: N^DIM lattices with
-// N a compile-time constant -- pure integer arithmetic, so the 2d rows and 2d links of a site are requested at once.
+// How a half-sweep finds its sites.  Tables: the orbit's order / fwd / bwd arrays, site by site (any all-even lattice;
+// three dependent global loads before the first row can be requested).  Cubic<N>: N^DIM lattices with N a compile-time
+// constant are walked block-wise by half_sweep_blocks() with pure integer arithmetic.
 template <int DIM>
 struct Tables {
-    static constexpr bool kPrefetch = false;   // locating a site costs dependent loads here
-    static constexpr int kBlocksN = 0;         // no block-wise half-sweep
+    static constexpr int kBlocksN = 0;   // no block-wise half-sweep
     __device__ static __forceinline__ void locate(const OrbitDev& D, int p, int r, int& i, int (&jf)[DIM], int (&jb)[DIM]) {
         i = __ldg(D.order + p * D.phase_off[1] + r);
 #pragma unroll
@@ -127,29 +122,8 @@ struct Tables {
 
 template <int DIM, int N>
 struct Cubic {
-    static constexpr bool kPrefetch = true;
-    static constexpr int kBlocksN = N;   // extent for the block-wise half-sweep
     static_assert(N % 2 == 0, "even extent");
-    __device__ static __forceinline__ void locate(const OrbitDev&, int p, int r, int& i, int (&jf)[DIM], int (&jb)[DIM]) {
-        // sites 2r and 2r+1 differ in x0 only (N even), so exactly one of them has parity p
-        int x[DIM], rest = 2 * r, s = 0;
-#pragma unroll
-        for (int mu = 0; mu < DIM; ++mu) {
-            x[mu] = rest % N;
-            rest /= N;
-            if (mu > 0) s += x[mu];
-        }
-        const int f = ((s & 1) != p) ? 1 : 0;
-        x[0] += f;
-        i = 2 * r + f;
-        int stride = 1;
-#pragma unroll
-        for (int mu = 0; mu < DIM; ++mu) {
-            jf[mu] = i + (x[mu] == N - 1 ? -(N - 1) * stride : stride);
-            jb[mu] = i + (x[mu] == 0 ? (N - 1) * stride : -stride);
-            stride *= N;
-        }
-    }
+    static constexpr int kBlocksN = N;   // extent for the block-wise half-sweep
 };
 
 // w_i = sum_mu [ conj(U_{i,mu}) g_{i+mu} + U_{i-mu,mu} g_{i-mu} ]   (= conj K_i of Eq. 5) for the start of
@@ -280,20 +254,6 @@ __device__ __forceinline__ double half_sweep_blocks(const OrbitDev& D, const dou
     return acc;
 }
 
-// Request the rows the NEXT site of this warp will read (its 2d neighbours and itself) into L1 while the current
-// site is computed: the half-sweep is otherwise bound by the L2 / HBM latency of one site per warp (ncu: long
-// scoreboard 5.8 stalled warps per issue).  Costs no registers; every lane touches its own 16 bytes of the row.
-template <int DIM>
-__device__ __forceinline__ void prefetch_rows(const double2* nb, const double2* own, int i, const int (&jf)[DIM],
-                                              const int (&jb)[DIM], int lane) {
-#pragma unroll
-    for (int mu = 0; mu < DIM; ++mu) {
-        asm volatile("prefetch.global.L1 [%0];" ::"l"(nb + (size_t)jf[mu] * 32 + lane));
-        asm volatile("prefetch.global.L1 [%0];" ::"l"(nb + (size_t)jb[mu] * 32 + lane));
-    }
-    asm volatile("prefetch.global.L1 [%0];" ::"l"(own + (size_t)i * 32 + lane));
-}
-
 template <int DIM, bool W1, class IDX>
 __global__ void __launch_bounds__(kThreads, 1) relax_stream_kernel(const StreamParams P) {
     constexpr unsigned FULL = 0xffffffffu;
@@ -398,10 +358,6 @@ __global__ void __launch_bounds__(kThreads, 1) relax_stream_kernel(const StreamP
             } else {
                 for (int r = warp; r < half; r += kWarps) {
                     int i, jf[DIM], jb[DIM];
-                    if (IDX::kPrefetch && kPrefetchAhead > 0 && r + kPrefetchAhead * kWarps < half) {
-                        IDX::locate(D, 1, r + kPrefetchAhead * kWarps, i, jf, jb);
-                        prefetch_rows<DIM>(E, A0, i, jf, jb, lane);
-                    }
                     IDX::locate(D, 1, r, i, jf, jb);
                     double wr, wi;
                     neighbour_sum<DIM>(D, E, i, jf, jb, lane, wr, wi);
@@ -433,10 +389,6 @@ __global__ void __launch_bounds__(kThreads, 1) relax_stream_kernel(const StreamP
             } else {
                 for (int r = warp; r < half; r += kWarps) {
                     int i, jf[DIM], jb[DIM];
-                    if (IDX::kPrefetch && kPrefetchAhead > 0 && r + kPrefetchAhead * kWarps < half) {
-                        IDX::locate(D, 0, r + kPrefetchAhead * kWarps, i, jf, jb);
-                        prefetch_rows<DIM>(A0, E, i, jf, jb, lane);
-                    }
                     IDX::locate(D, 0, r, i, jf, jb);
                     double wr, wi;
                     neighbour_sum<DIM>(D, A0, i, jf, jb, lane, wr, wi);
