@@ -96,7 +96,7 @@ int u1gf_relax_batch_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_sta
                           double* sig_host, double* g_canon_host);
 
 /* Kernel selection for u1gf_relax_batch on this handle: 0 = automatic (specialised resident kernel when one
- * exists for the extents; the streamed lane-per-start kernel for all-even lattices of 512 sites and more and its
+ * exists for the extents; the streamed lane-per-start kernel for all-even lattices of 1024 sites and more and its
  * phased variant for lattices with an odd extent of 64 sites and more; else the generic one), 1 = force the generic
  * kernel, 2 = force the streamed / phased lane-per-start kernel.
  * Results per start are the same copies either way; kernels may differ in the last bits of F and, rarely, by a

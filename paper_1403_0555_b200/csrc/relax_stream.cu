@@ -678,10 +678,12 @@ int launch(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st) {
 // every extent even (two-colour checkerboard); chosen automatically from 512 sites up, where a team's field no longer
 // fits on chip and the generic kernel's per-start link traffic dominates
 bool stream_supported(const u1gf_orbit* o) { return o->dev.d >= 1 && o->dev.d <= 4; }
-// automatic choice: all-even lattices from 512 sites up (the fused two-colour kernel), lattices with an odd extent from
-// 64 sites up (the phased kernel; 3^4 = 81)
+// automatic choice: all-even lattices from 1024 sites up (the fused two-colour kernel; measured against the generic
+// kernel: 6^4 302 vs 732 ms, 8^4 960 vs 1777 ms, but 8^3 41 vs 29 ms and 12^2 14 vs 13 ms -- below about a thousand
+// sites the two barriers per sweep outweigh the shared link reads), lattices with an odd extent from 64 sites up (the
+// phased kernel; 3^4 = 81: 87 vs 320 ms)
 bool stream_preferred(const u1gf_orbit* o) {
-    return stream_supported(o) && (o->dev.all_even ? o->dev.V >= 512 : o->dev.V >= 64);
+    return stream_supported(o) && (o->dev.all_even ? o->dev.V >= 1024 : o->dev.V >= 64);
 }
 
 size_t stream_workspace_bytes(const u1gf_orbit* o, uint64_t n) {
