@@ -343,3 +343,26 @@ def test_discovery_curve_and_paper_count_match_oracle(b, oracle):
     assert _cpu(b.discovery_curve(torch.zeros(1, dtype=torch.int64, device="cuda"), 0, 4)).tolist() == [0, 0, 0, 0]
     with pytest.raises(b.U1gfError):
         b.discovery_curve(torch.zeros(1, dtype=torch.int64, device="cuda"), 1, 66)
+
+
+@pytest.mark.gpu
+def test_omega_changes_basins_not_copies_on_gpu(b):
+    """SURVEY 8(f)-2 / pin P12 at GPU scale: omega = 1 (the paper's relaxation) and omega = 1.7 find the
+    same copies on saturated small orbits (the set of F/(dV) values agrees to 1e-9) while the start -> copy map and
+    the multiplicities differ (on these tiny lattices plain relaxation even needs fewer sweeps)."""
+    import torch
+    for ext, seed, n in (((4, 4), 1, 1 << 16), ((2, 2, 2, 2), 12, 1 << 16)):
+        orbit = b.Orbit(ext, synth.uniform_links(ext, seed))
+        tables = {}
+        for omega in (1.0, 1.7):
+            r = b.relax_batch(orbit, seed, n, omega=omega)
+            c = b.count_copies(r["F_norm"], r["sig"], r["status"])
+            nd = int(c["n_distinct"].item())
+            F = np.sort(_cpu(r["F_norm"])[_cpu(c["rep"])[:nd]])
+            tables[omega] = (F, _cpu(c["copy_id"]), float(r["sweeps"].float().mean().item()), np.sort(_cpu(c["multiplicity"])[:nd]))
+            assert int((r["status"] & 1).sum().item()) == 0
+        F1, id1, sw1, m1 = tables[1.0]
+        F17, id17, sw17, m17 = tables[1.7]
+        assert F1.size == F17.size and np.abs(F1 - F17).max() < 1e-9
+        assert sw1 != sw17                                 # a different path to the same copies ...
+        assert (m1 != m17).any()                           # ... into basins of different sizes (the bias of L99)
