@@ -48,7 +48,7 @@ LATTICES = [
     ((4, 4), 1, 512), ((8, 8), 2, 256), ((4, 4, 4), 3, 256), ((4, 4, 4, 4), 12, 96), ((2, 2, 2, 2), 12, 512),
     ((3, 3, 3, 3), 12, 128), ((3, 2), 40, 256), ((2, 2), 41, 256), ((5, 3, 2), 7, 128), ((6, 6, 6, 6), 12, 12),
     ((8, 8, 8, 8), 12, 4), ((7,), 77, 128), ((6, 4), 5, 128), ((4, 6, 2, 3), 9, 32), ((10, 10), 8, 64),
-    ((8, 8, 8), 21, 70), ((6, 6), 22, 300),
+    ((8, 8, 8), 21, 70), ((6, 6), 22, 300), ((6, 6, 6), 23, 40),
 ]
 
 
