@@ -366,3 +366,29 @@ def test_omega_changes_basins_not_copies_on_gpu(b):
         assert F1.size == F17.size and np.abs(F1 - F17).max() < 1e-9
         assert sw1 != sw17                                 # a different path to the same copies ...
         assert (m1 != m17).any()                           # ... into basins of different sizes (the bias of L99)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("ext,seed,n,kind", [
+    ((4, 4, 4, 4), 12, 1 << 17, "uniform"), ((4, 4, 4, 4), 11, 1 << 17, "gauss0.8"), ((4, 4, 4), 3, 1 << 18, "uniform"),
+    ((8, 8), 2, 1 << 18, "gauss0.6"), ((2, 2, 2, 2), 12, 1 << 18, "uniform"), ((4, 4), 1, 1 << 18, "uniform"),
+    ((6, 6, 6, 6), 12, 1 << 12, "uniform"), ((3, 3, 3, 3), 12, 1 << 16, "uniform"), ((8, 8, 8, 8), 12, 1 << 9, "uniform")])
+def test_large_batches_element_by_element(b, oracle, ext, seed, n, kind):
+    """Every start of a large batch against the oracle (10^5 .. 3 10^5 starts on the resident kernels, thousands on the
+    big lattices): identical sweeps and status, F/(dV) within 1e-10, and the same copy id for every start -- up to 6 10^4
+    distinct copies on the hot 4^4 orbit.  This is where a rounding-level difference between the two arithmetic paths
+    (FMA contraction, second-order rsqrt polish, tree gauge, summation order) would show up as a sweep or a copy (R14)."""
+    th = synth.uniform_links(ext, seed) if kind == "uniform" else synth.gaussian_gauged_links(ext, seed, float(kind[5:]))
+    orbit = b.Orbit(ext, th)
+    eps = 1e-12 if orbit.V > 256 else 1e-13
+    o = oracle.relax(ext, th, seed, n, eps=eps)
+    r = b.relax_batch(orbit, seed, n, eps=eps)
+    sw, F, st, sg = (_cpu(r[k]) for k in ("sweeps", "F_norm", "status", "sig"))
+    bad = np.nonzero(sw != o["sweeps"])[0]
+    assert bad.size == 0, f"sweeps differ at starts {bad[:10]}: oracle {o['sweeps'][bad[:10]]} gpu {sw[bad[:10]]}"
+    assert (st == o["status"]).all()
+    assert np.abs(F - o["F_norm"]).max() < TOL_F and np.abs(sg - o["sig"]).max() < TOL_G
+    c = b.count_copies(r["F_norm"], r["sig"], r["status"])
+    oc = oracle.count_copies(o["F_norm"], o["sig"], o["status"])
+    assert int(c["n_distinct"].item()) == oc["n_distinct"]
+    assert (_cpu(c["copy_id"]) == oc["copy_id"]).all()
