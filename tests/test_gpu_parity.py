@@ -392,3 +392,23 @@ def test_large_batches_element_by_element(b, oracle, ext, seed, n, kind):
     oc = oracle.count_copies(o["F_norm"], o["sig"], o["status"])
     assert int(c["n_distinct"].item()) == oc["n_distinct"]
     assert (_cpu(c["copy_id"]) == oc["copy_id"]).all()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("ext,seed,n", [((4, 4, 4, 4), 12, 1200), ((4, 4, 4), 3, 4000), ((6, 6, 6, 6), 12, 24), ((3, 3, 3, 3), 12, 600)])
+def test_check_fp_every_copy_of_a_batch(b, oracle, ext, seed, n):
+    """a7 on every distinct copy of a hot batch (about 1000 copies at 4^4): lambda_1 of the batched Lanczos kernel against
+    the oracle's dense eigenvalue within 1e-8 (observed: 1e-13), identical region flags."""
+    th = synth.uniform_links(ext, seed)
+    orbit = b.Orbit(ext, th)
+    eps = 1e-12 if orbit.V > 256 else 1e-13
+    r = b.relax_batch(orbit, seed, n, eps=eps, want_g=True)
+    c = b.count_copies(r["F_norm"], r["sig"], r["status"])
+    nd = int(c["n_distinct"].item())
+    g = r["g_canon"][c["rep"][:nd]].contiguous()
+    f = b.check_fp(orbit, g)
+    lam, reg, gh = _cpu(f["lambda1"]), _cpu(f["region"]), _cpu(g)
+    for k in range(nd):
+        lo, ro = oracle.fp_lambda1(ext, th, gh[k])
+        assert abs(lo - lam[k]) < 1e-8 and ro == reg[k], f"copy {k}: oracle {lo} gpu {lam[k]}"
+    assert int(f["n_in_region"].item()) == int((reg != 0).sum())
