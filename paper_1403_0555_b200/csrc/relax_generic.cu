@@ -24,6 +24,10 @@ struct Params {
     double* sig;
     double* g_canon;
     unsigned long long* counter;
+    // redo mode (R6 fix-up of the resident kernels): the number of starts comes from device memory and entry idx of the
+    // work list is the position pos[idx] in the output arrays (and in start_ids); both NULL otherwise
+    const unsigned* n_dev;
+    const unsigned long long* pos;
 };
 
 // w_i = sum_mu [ conj(U_{i,mu}) g_{i+mu} + U_{i-mu,mu} g_{i-mu} ]   (= conj K_i of Eq. 5)
@@ -103,8 +107,9 @@ __global__ void __launch_bounds__(1024) relax_generic_kernel(const OrbitDev D, c
     for (;;) {
         if (tid == 0) s_next = atomicAdd(P.counter, 1ull);
         __syncthreads();
-        const unsigned long long k = s_next;
-        if (k >= P.n_starts) break;
+        unsigned long long k = s_next;
+        if (k >= (P.n_dev ? (unsigned long long)*P.n_dev : P.n_starts)) break;
+        if (P.pos) k = P.pos[k];
         const uint64_t s = P.start_ids ? P.start_ids[k] : P.first_start + k;
 
         // a2: random start
@@ -253,7 +258,7 @@ Launch pick(const u1gf_orbit* o) {
 }
 
 template <int DIM, int MAXS>
-int launch(const u1gf_orbit* o, const Params& P, int T, cudaStream_t st) {
+int launch(const u1gf_orbit* o, const Params& P, int T, cudaStream_t st, bool redo = false) {
     auto kern = relax_generic_kernel<DIM, MAXS>;
     const size_t smem = (size_t)o->dev.V * sizeof(double2);
     if (smem > 48 * 1024) U1GF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -262,6 +267,12 @@ int launch(const u1gf_orbit* o, const Params& P, int T, cudaStream_t st) {
     if (per_sm < 1) return fail(U1GF_ECUDA, "generic relaxation kernel does not fit on an SM (V = %d)", o->dev.V);
     unsigned long long grid = (unsigned long long)per_sm * (unsigned long long)o->sm_count;
     if (grid > P.n_starts) grid = P.n_starts;
+    if (redo) {   // the caller zeroed the counter and brackets the whole call with its own events
+        kern<<<(unsigned)grid, T, smem, st>>>(o->dev, P);
+        U1GF_CUDA(cudaGetLastError());
+        ++t_launches;
+        return U1GF_OK;
+    }
     U1GF_CUDA(cudaMemsetAsync(P.counter, 0, sizeof(unsigned long long), st));
     U1GF_CUDA(cudaEventRecord(t_ev0, st));
     kern<<<(unsigned)grid, T, smem, st>>>(o->dev, P);
@@ -273,11 +284,11 @@ int launch(const u1gf_orbit* o, const Params& P, int T, cudaStream_t st) {
 }
 
 template <int DIM>
-int launch_d(const u1gf_orbit* o, const Params& P, Launch L, cudaStream_t st) {
+int launch_d(const u1gf_orbit* o, const Params& P, Launch L, cudaStream_t st, bool redo = false) {
     switch (L.maxs) {
-        case 1: return launch<DIM, 1>(o, P, L.T, st);
-        case 2: return launch<DIM, 2>(o, P, L.T, st);
-        default: return launch<DIM, 4>(o, P, L.T, st);
+        case 1: return launch<DIM, 1>(o, P, L.T, st, redo);
+        case 2: return launch<DIM, 2>(o, P, L.T, st, redo);
+        default: return launch<DIM, 4>(o, P, L.T, st, redo);
     }
 }
 
@@ -285,9 +296,24 @@ int launch_d(const u1gf_orbit* o, const Params& P, Launch L, cudaStream_t st) {
 
 size_t generic_workspace_bytes(const u1gf_orbit*, uint64_t) { return 256; }
 
+int generic_relax_list(const u1gf_orbit* o, const RelaxArgs& a, const unsigned* n_dev, const unsigned long long* pos,
+                       unsigned long long* counter, cudaStream_t st) {
+    Params P{a.seed, a.first_start, a.n_starts, a.start_ids, a.omega, a.eps, a.max_sweeps, a.check_every,
+             a.F_norm, a.sweeps, a.status, a.sig, a.g_canon, counter, n_dev, pos};
+    // a small grid: the list is empty unless a neighbour sum vanished somewhere (R6)
+    if (P.n_starts > 4ull * (unsigned long long)o->sm_count) P.n_starts = 4ull * (unsigned long long)o->sm_count;
+    const Launch L = pick(o);
+    switch (o->dev.d) {
+        case 1: return launch_d<1>(o, P, L, st, true);
+        case 2: return launch_d<2>(o, P, L, st, true);
+        case 3: return launch_d<3>(o, P, L, st, true);
+        default: return launch_d<4>(o, P, L, st, true);
+    }
+}
+
 int generic_relax(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st) {
     Params P{a.seed, a.first_start, a.n_starts, a.start_ids, a.omega, a.eps, a.max_sweeps, a.check_every,
-             a.F_norm, a.sweeps, a.status, a.sig, a.g_canon, (unsigned long long*)a.workspace};
+             a.F_norm, a.sweeps, a.status, a.sig, a.g_canon, (unsigned long long*)a.workspace, nullptr, nullptr};
     const Launch L = pick(o);
     switch (o->dev.d) {
         case 1: return launch_d<1>(o, P, L, st);

@@ -131,6 +131,10 @@ struct RelaxArgs {
 
 size_t generic_workspace_bytes(const u1gf_orbit* o, uint64_t n);
 int generic_relax(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st);
+// redo mode: relax the starts at output positions pos[0 .. *n_dev) again (R6 fix-up of the resident kernels); `counter` is a
+// zeroed device word; no events are recorded
+int generic_relax_list(const u1gf_orbit* o, const RelaxArgs& a, const unsigned* n_dev, const unsigned long long* pos,
+                       unsigned long long* counter, cudaStream_t st);
 
 // specialised "lane per start" resident kernels; lanes_supported() says whether the extents have one
 bool lanes_supported(const u1gf_orbit* o);
