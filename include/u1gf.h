@@ -41,7 +41,7 @@ typedef struct u1gf_orbit u1gf_orbit; /* opaque, library-owned */
 
 const char* u1gf_last_error(void);
 
-/* Version of this ABI (bumped on incompatible change). */
+/* Version of this ABI (bumped on incompatible change; 2 = round 2: ensembles, pipeline, region bit 2). */
 int u1gf_abi_version(void);
 
 /* ---------------------------------------------------------------------------------------------------------
@@ -112,12 +112,17 @@ const char* u1gf_kernel_name(const u1gf_orbit* o);
  * the orthogonal complement of the constant vector (the global gauge zero mode), computed by a
  * batched matrix-free Lanczos iteration (one CTA per configuration).
  *   g           dev [n_cfg*V*2]
- *   tol_fp      region = 1 if lambda_1 > tol_fp (inside), 2 if |lambda_1| <= tol_fp (marginal, "semi"definite),
- *               0 if lambda_1 < -tol_fp (outside)
- *   lambda1     dev [n_cfg];  region dev [n_cfg];  n_in_region dev [1] = number of configurations with region != 0
+ *   tol_fp      region bits 0-1 = 1 if lambda_1 > tol_fp (inside), 2 if |lambda_1| <= tol_fp (marginal, "semi"definite),
+ *               0 if lambda_1 < -tol_fp (outside); region bit 2 (value 4) is set when the iteration reached its cap of
+ *               min(V-1, 512) steps with the Ritz residual bound still above 1e-10 (R16): lambda1 is then only an upper
+ *               bound of the eigenvalue, and an "inside" verdict is not proven
+ *   lambda1     dev [n_cfg];  region dev [n_cfg];  n_in_region dev [1] = number of configurations with (region & 3) != 0
+ *   lanczos_steps  dev [n_cfg] int32 or NULL: Lanczos steps taken per configuration
+ * A converged relaxation can stop at a saddle it is still leaving (the stop rule tests the gradient only):
+ * such copies come out with region 0 and are genuine -- DESIGN.md section 3, R17.
  * ------------------------------------------------------------------------------------------------------- */
 int u1gf_check_fp(const u1gf_orbit* o, uint64_t n_cfg, const double* g, double tol_fp, double* lambda1,
-                  uint8_t* region, int64_t* n_in_region, void* cuda_stream);
+                  uint8_t* region, int64_t* n_in_region, int32_t* lanczos_steps, void* cuda_stream);
 int u1gf_check_fp_host(const u1gf_orbit* o, uint64_t n_cfg, const double* g_host, double tol_fp,
                        double* lambda1_host, uint8_t* region_host, int64_t* n_in_region_host);
 
@@ -168,32 +173,75 @@ int u1gf_paper_count(uint64_t n, const double* F_norm, const uint8_t* status, do
                      void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------------------
- * Measurement helpers (not part of the method): roofline denominators measured on the device in use.
- *   u1gf_measure_fp64_peak   runs a dependent-chain-free DFMA kernel on all SMs for about `ms` milliseconds and
- *                            returns FP64 FMA instructions (thread-level) per second in *dfma_per_s.
- *   u1gf_measure_fp64_rate   the same rate for a DFMA stream of a given operand pattern: 0 = the stream of
- *                            u1gf_measure_fp64_peak (one register operand, two constants); 1 = three distinct
- *                            register operands per DFMA; 2 = the complex multiply-accumulate pattern of the
- *                            neighbour sum w_i (Eq. 5); 3 / 4 = stream 0 / stream 1 with two independent
- *                            integer instructions per DFMA (FP64 FMAs counted only); 5 = one dependent chain per
- *                            warp, one warp per scheduler (rate = threads in flight / dependent-issue latency);
- *                            6 = FP64 tensor-core DMMA m8n8k4, 8 FMAs per thread and instruction.  Patterns 1-4
- *                            are limited by register-file operand bandwidth, not by the FP64 lanes.
- *   u1gf_measure_smem_rate   warp-level shared-memory instructions per second of a mix: 0 = 4 lane-strided LDS.128
- *                            + 1 STS.128 (neighbours of 32 starts and the store), 1 = 8 warp-uniform LDS.128
- *                            (links), 2 = both (the 13 shared-memory instructions of one 4^4 site update).
- *   u1gf_measure_smem_peak   same for 128-bit conflict-free shared-memory loads, bytes per second.
- *   u1gf_last_launch_count   kernels launched by the calling thread's most recent compute call.
- *   u1gf_last_relax_ms       device time (CUDA events on the call's stream) of the relaxation kernel of the
- *                            calling thread's most recent u1gf_relax_batch*, after synchronising those events;
- *                            returns < 0 if none.
+ * The whole hot path in one call with HOST result buffers (what an application that keeps nothing on the device
+ * calls, and what bench.py's `e2e` times): u1gf_relax_batch on all starts -> u1gf_count_copies -> the representatives
+ * re-relaxed with their fields -> u1gf_check_fp.  Intermediates never leave the device; device scratch comes from a
+ * grow-only per-thread allocation that is kept between calls (u1gf_release_host_scratch frees it; the other *_host
+ * calls use the same scratch).
+ *   per start (host [n_starts] or NULL): F_norm, sweeps, status, sig [n*4], copy_id
+ *   per copy  (host arrays of copy_capacity entries or NULL): rep (position of the leader), multiplicity, F_rep
+ *             (F/(dV) of the leader), lambda1, region (as u1gf_check_fp); U1GF_ENOMEM if n_distinct > copy_capacity
+ *             and any per-copy array is given
+ *   n_distinct [1], n_in_region [1] (host, required); hist host [nbins] or NULL
  * ------------------------------------------------------------------------------------------------------- */
-int u1gf_measure_fp64_peak(double ms, double* dfma_per_s, void* cuda_stream);
-int u1gf_measure_fp64_rate(int32_t pattern, double ms, double* dfma_per_s, void* cuda_stream);
-int u1gf_measure_smem_peak(double ms, double* bytes_per_s, void* cuda_stream);
-int u1gf_measure_smem_rate(int32_t mix, double ms, double* instr_per_s, void* cuda_stream);
-int32_t u1gf_last_launch_count(void);
-double u1gf_last_relax_ms(void);
+int u1gf_pipeline_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_start, uint64_t n_starts, double omega,
+                       double eps, int32_t max_sweeps, int32_t check_every, double tol_F, double tol_sig, double tol_fp,
+                       int32_t nbins, double* F_norm_host, int32_t* sweeps_host, uint8_t* status_host, double* sig_host,
+                       int32_t* copy_id_host, int64_t copy_capacity, int64_t* n_distinct_host, int64_t* rep_host,
+                       int64_t* multiplicity_host, double* F_rep_host, double* lambda1_host, uint8_t* region_host,
+                       int64_t* n_in_region_host, int64_t* hist_host);
+int u1gf_release_host_scratch(void);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Ensembles: many gauge orbits of ONE lattice shape relaxed in ONE kernel launch.  The paper's
+ * workload is an ensemble -- 100 orbits x 4 mebisamples per lattice size (Tab. I, Tab. III),
+ * one lattice per thread block, grid over the samples (L121).
+ *   u1gf_create_ensemble   theta_host [n_orbits][V*d] link angles, seeds_host [n_orbits] start seed of each orbit
+ *                          (starts of orbit o are those of u1gf_relax_batch with seed seeds[o]).  Only lattice shapes
+ *                          with a resident kernel (4x4, 8x8, 4^3, 2^4, 4^4), else U1GF_EINVAL.  Synchronous.
+ *   u1gf_ensemble_orbit    member k as an ordinary orbit handle (owned by the ensemble): for u1gf_check_fp and for
+ *                          re-relaxing an orbit's representatives with u1gf_relax_batch(start_ids, g_canon)
+ *   u1gf_relax_ensemble    every orbit runs the starts first_start + [0, n_starts_per_orbit); result k of orbit o is at
+ *                          o * n_starts_per_orbit + k of F_norm / sweeps / status / sig [.*4] (device arrays of
+ *                          n_orbits * n_starts_per_orbit entries).  Per start the results are those of
+ *                          u1gf_relax_batch on the member orbit, with one exception: a start that meets R6
+ *                          (|w|^2 < 1e-280) comes back with status 3 instead of being relaxed with the skip rule.
+ *   u1gf_count_copies_ensemble   u1gf_count_copies per orbit on those arrays: copy ids, rep (positions) and
+ *                          multiplicity are local to the orbit and stored at o * n_per_orbit; n_distinct dev
+ *                          [n_orbits]; hist dev [n_orbits * nbins] or NULL; workspace >= u1gf_count_workspace_bytes(n_per_orbit)
+ * ------------------------------------------------------------------------------------------------------- */
+typedef struct u1gf_ensemble u1gf_ensemble; /* opaque, library-owned */
+int u1gf_create_ensemble(int d, const int32_t* extents, int32_t n_orbits, const double* theta_host,
+                         const uint64_t* seeds_host, u1gf_ensemble** out);
+int u1gf_destroy_ensemble(u1gf_ensemble* e);
+int32_t u1gf_ensemble_size(const u1gf_ensemble* e);
+const u1gf_orbit* u1gf_ensemble_orbit(const u1gf_ensemble* e, int32_t k);
+size_t u1gf_relax_ensemble_workspace_bytes(const u1gf_ensemble* e, uint64_t n_starts_per_orbit);
+int u1gf_relax_ensemble(const u1gf_ensemble* e, uint64_t first_start, uint64_t n_starts_per_orbit, double omega,
+                        double eps, int32_t max_sweeps, int32_t check_every, double* F_norm, int32_t* sweeps,
+                        uint8_t* status, double* sig, void* workspace, size_t workspace_bytes, void* cuda_stream);
+size_t u1gf_count_ensemble_workspace_bytes(uint64_t n_per_orbit);
+int u1gf_count_copies_ensemble(int32_t n_orbits, uint64_t n_per_orbit, const double* F_norm, const double* sig,
+                               const uint8_t* status, double tol_F, double tol_sig, int32_t* copy_id,
+                               int64_t* n_distinct, int64_t* rep, int64_t* multiplicity, int64_t* hist, int32_t nbins,
+                               void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Merging the copy tables of several start ranges (the paper runs 4 GPUs on independent samples,
+ * PAPER.md:L121).  Each range was de-duplicated on its own; entry e of the concatenated tables is one copy of one
+ * range: F_rep[e] = F/(dV) of its leader, sig_rep[e*4..], first_start[e] = GLOBAL start index of its leader,
+ * multiplicity[e].  The entries are ordered by first_start (the discovery order of the whole job, L149) and clustered by
+ * the copy identity of u1gf_count_copies (R7).  Outputs: merged_id[e] = merged copy of entry e, merged copies numbered
+ * by increasing first discovery; n_merged dev [1]; merged_first_start / merged_multiplicity dev [m], the first n_merged
+ * entries valid.  The global copy id of a start is merged_id[offset of its range + its local copy id].
+ * All arrays dev, int64 unless stated; workspace >= u1gf_merge_workspace_bytes(m), 256-byte aligned; asynchronous.
+ * ------------------------------------------------------------------------------------------------------- */
+size_t u1gf_merge_workspace_bytes(uint64_t m);
+int u1gf_merge_copy_tables(uint64_t m, const double* F_rep, const double* sig_rep, const int64_t* first_start,
+                           const int64_t* multiplicity, double tol_F, double tol_sig, int32_t* merged_id,
+                           int64_t* n_merged, int64_t* merged_first_start, int64_t* merged_multiplicity,
+                           void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 
 #ifdef __cplusplus
 }

@@ -29,7 +29,7 @@ _SIGNATURES = {
                                         C.c_int32, C.c_int32, _p, _p, _p, _p, _p]),
     "u1gf_set_kernel": (C.c_int, [_p, C.c_int32]),
     "u1gf_kernel_name": (C.c_char_p, [_p]),
-    "u1gf_check_fp": (C.c_int, [_p, C.c_uint64, _p, C.c_double, _p, _p, _p, _p]),
+    "u1gf_check_fp": (C.c_int, [_p, C.c_uint64, _p, C.c_double, _p, _p, _p, _p, _p]),
     "u1gf_check_fp_host": (C.c_int, [_p, C.c_uint64, _p, C.c_double, _p, _p, _p]),
     "u1gf_count_workspace_bytes": (C.c_size_t, [C.c_uint64]),
     "u1gf_count_copies": (C.c_int, [C.c_uint64, _p, _p, _p, C.c_double, C.c_double, _p, _p, _p, _p, _p, C.c_int32,
@@ -39,15 +39,38 @@ _SIGNATURES = {
     "u1gf_discovery_curve": (C.c_int, [C.c_uint64, _p, C.c_int32, _p, _p]),
     "u1gf_paper_count_workspace_bytes": (C.c_size_t, [C.c_uint64]),
     "u1gf_paper_count": (C.c_int, [C.c_uint64, _p, _p, C.c_double, _p, _p, C.c_size_t, _p]),
+    "u1gf_pipeline_host": (C.c_int, [_p, C.c_uint64, C.c_uint64, C.c_uint64, C.c_double, C.c_double, C.c_int32, C.c_int32,
+                                     C.c_double, C.c_double, C.c_double, C.c_int32, _p, _p, _p, _p, _p, C.c_int64, _p, _p,
+                                     _p, _p, _p, _p, _p, _p]),
+    "u1gf_release_host_scratch": (C.c_int, []),
+    "u1gf_create_ensemble": (C.c_int, [C.c_int, _p, C.c_int32, _p, _p, C.POINTER(_p)]),
+    "u1gf_destroy_ensemble": (C.c_int, [_p]),
+    "u1gf_ensemble_size": (C.c_int32, [_p]),
+    "u1gf_ensemble_orbit": (_p, [_p, C.c_int32]),
+    "u1gf_relax_ensemble_workspace_bytes": (C.c_size_t, [_p, C.c_uint64]),
+    "u1gf_relax_ensemble": (C.c_int, [_p, C.c_uint64, C.c_uint64, C.c_double, C.c_double, C.c_int32, C.c_int32, _p, _p, _p,
+                                      _p, _p, C.c_size_t, _p]),
+    "u1gf_count_ensemble_workspace_bytes": (C.c_size_t, [C.c_uint64]),
+    "u1gf_count_copies_ensemble": (C.c_int, [C.c_int32, C.c_uint64, _p, _p, _p, C.c_double, C.c_double, _p, _p, _p, _p, _p,
+                                             C.c_int32, _p, C.c_size_t, _p]),
+    "u1gf_merge_workspace_bytes": (C.c_size_t, [C.c_uint64]),
+    "u1gf_merge_copy_tables": (C.c_int, [C.c_uint64, _p, _p, _p, _p, C.c_double, C.c_double, _p, _p, _p, _p, _p,
+                                         C.c_size_t, _p]),
+}
+
+# include/u1gf_measure.h: one symbol of libu1gf.so and the probes of libu1gf_measure.so
+_MEASURE_SIGNATURES_MAIN = {"u1gf_last_launch_count": (C.c_int32, [])}
+_MEASURE_SIGNATURES = {
+    "u1gf_measure_last_error": (C.c_char_p, []),
     "u1gf_measure_fp64_peak": (C.c_int, [C.c_double, C.POINTER(C.c_double), _p]),
     "u1gf_measure_fp64_rate": (C.c_int, [C.c_int32, C.c_double, C.POINTER(C.c_double), _p]),
     "u1gf_measure_smem_peak": (C.c_int, [C.c_double, C.POINTER(C.c_double), _p]),
     "u1gf_measure_smem_rate": (C.c_int, [C.c_int32, C.c_double, C.POINTER(C.c_double), _p]),
-    "u1gf_last_launch_count": (C.c_int32, []),
-    "u1gf_last_relax_ms": (C.c_double, []),
 }
+MEASURE_LIB_PATH = os.path.join(_HERE, "libu1gf_measure.so")
 
 _lib = None
+_mlib = None
 
 
 class U1gfError(RuntimeError):
@@ -63,7 +86,7 @@ def lib():
         if not os.path.exists(LIB_PATH):
             raise FileNotFoundError(f"{LIB_PATH} not built; run `python -m paper_1403_0555_b200.build`")
         L = C.CDLL(LIB_PATH)
-        for name, (res, args) in _SIGNATURES.items():
+        for name, (res, args) in {**_SIGNATURES, **_MEASURE_SIGNATURES_MAIN}.items():
             fn = getattr(L, name)
             fn.restype = res
             fn.argtypes = args
@@ -71,8 +94,35 @@ def lib():
     return _lib
 
 
+def use_library(path):
+    """Load another build of the method library (tests: build.build_variant) in place of libu1gf.so."""
+    global _lib, LIB_PATH
+    LIB_PATH = path
+    _lib = None
+    return lib()
+
+
+def measure_lib():
+    """Load libu1gf_measure.so (include/u1gf_measure.h: roofline probes, not the method)."""
+    global _mlib
+    if _mlib is None:
+        if not os.path.exists(MEASURE_LIB_PATH):
+            raise FileNotFoundError(f"{MEASURE_LIB_PATH} not built; run `python -m paper_1403_0555_b200.build`")
+        L = C.CDLL(MEASURE_LIB_PATH)
+        for name, (res, args) in _MEASURE_SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _mlib = L
+    return _mlib
+
+
 def exported_symbols():
     return sorted(_SIGNATURES)
+
+
+def measure_symbols():
+    return sorted({**_MEASURE_SIGNATURES_MAIN, **_MEASURE_SIGNATURES})
 
 
 def _check(rc):
@@ -109,6 +159,9 @@ class Orbit:
         self.V = int(np.prod(e))
 
     def close(self):
+        if getattr(self, "_borrowed", False):   # a member of an Ensemble: the ensemble frees it
+            self.handle = None
+            return
         if getattr(self, "handle", None):
             lib().u1gf_destroy_orbit(self.handle)
             self.handle = None
@@ -125,6 +178,122 @@ class Orbit:
     @property
     def kernel_name(self) -> str:
         return lib().u1gf_kernel_name(self.handle).decode()
+
+
+class Ensemble:
+    """u1gf_ensemble handle: n_orbits orbits of one lattice shape relaxed in one launch."""
+
+    def __init__(self, extents, thetas, seeds):
+        ext = np.ascontiguousarray(extents, dtype=np.int32)
+        th = np.ascontiguousarray(thetas, dtype=np.float64)
+        sd = np.ascontiguousarray(seeds, dtype=np.uint64)
+        self.extents = tuple(int(e) for e in ext)
+        self.d, self.V, self.n_orbits = ext.size, int(np.prod(ext)), int(sd.size)
+        assert th.size == self.n_orbits * self.V * self.d, "thetas must be [n_orbits][V*d]"
+        h = C.c_void_p()
+        _check(lib().u1gf_create_ensemble(self.d, _np_ptr(ext), self.n_orbits, _np_ptr(th), _np_ptr(sd), C.byref(h)))
+        self.handle = h
+        self.seeds = sd
+
+    def orbit(self, k):
+        """Member k as an Orbit (borrowed: the ensemble owns it)."""
+        o = Orbit.__new__(Orbit)
+        o.extents, o.d, o.V = self.extents, self.d, self.V
+        o.handle = C.c_void_p(lib().u1gf_ensemble_orbit(self.handle, int(k)))
+        o._borrowed = True
+        return o
+
+    def close(self):
+        if getattr(self, "handle", None):
+            _check(lib().u1gf_destroy_ensemble(self.handle))
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def relax_ensemble(ens: Ensemble, n_starts_per_orbit, *, first_start=0, omega=1.7, eps=1e-13, max_sweeps=20000,
+                   check_every=1, workspace=None):
+    """u1gf_relax_ensemble -> dict of device tensors shaped [n_orbits, n] (sig [n_orbits, n, 4])."""
+    import torch
+    n, no = int(n_starts_per_orbit), ens.n_orbits
+    out = dict(F_norm=torch.empty((no, n), dtype=torch.float64, device="cuda"),
+               sweeps=torch.empty((no, n), dtype=torch.int32, device="cuda"),
+               status=torch.empty((no, n), dtype=torch.uint8, device="cuda"),
+               sig=torch.empty((no, n, 4), dtype=torch.float64, device="cuda"))
+    need = lib().u1gf_relax_ensemble_workspace_bytes(ens.handle, n)
+    if workspace is None or workspace.numel() < need + 256:
+        workspace = _workspace(need)
+    out["workspace"] = workspace
+    _check(lib().u1gf_relax_ensemble(ens.handle, int(first_start), n, float(omega), float(eps), int(max_sweeps),
+                                     int(check_every), _dev_ptr(out["F_norm"]), _dev_ptr(out["sweeps"]),
+                                     _dev_ptr(out["status"]), _dev_ptr(out["sig"]), _aligned_ptr(workspace), need, _stream()))
+    return out
+
+
+def count_copies_ensemble(F_norm, sig, status, tol_F=1e-10, tol_sig=1e-4, nbins=0, workspace=None):
+    """u1gf_count_copies_ensemble on [n_orbits, n] device tensors -> per-orbit tables ([n_orbits, n], n_distinct [n_orbits])."""
+    import torch
+    no, n = int(F_norm.shape[0]), int(F_norm.shape[1])
+    copy_id = torch.empty((no, n), dtype=torch.int32, device="cuda")
+    nd = torch.zeros(no, dtype=torch.int64, device="cuda")
+    rep = torch.empty((no, max(n, 1)), dtype=torch.int64, device="cuda")
+    mult = torch.empty((no, max(n, 1)), dtype=torch.int64, device="cuda")
+    hist = torch.empty((no, nbins), dtype=torch.int64, device="cuda") if nbins else None
+    need = lib().u1gf_count_ensemble_workspace_bytes(n)
+    if workspace is None or workspace.numel() < need + 256:
+        workspace = _workspace(need)
+    _check(lib().u1gf_count_copies_ensemble(no, n, _dev_ptr(F_norm), _dev_ptr(sig), _dev_ptr(status), float(tol_F),
+                                            float(tol_sig), _dev_ptr(copy_id), _dev_ptr(nd), _dev_ptr(rep), _dev_ptr(mult),
+                                            _dev_ptr(hist), int(nbins), _aligned_ptr(workspace), need, _stream()))
+    return dict(copy_id=copy_id, n_distinct=nd, rep=rep, multiplicity=mult, hist=hist, workspace=workspace)
+
+
+def merge_copy_tables(F_rep, sig_rep, first_start, multiplicity, tol_F=1e-10, tol_sig=1e-4):
+    """u1gf_merge_copy_tables on device tensors -> dict(merged_id, n_merged, first_start, multiplicity)."""
+    import torch
+    m = int(F_rep.numel())
+    mid = torch.empty(m, dtype=torch.int32, device="cuda")
+    nm = torch.zeros(1, dtype=torch.int64, device="cuda")
+    mfs = torch.empty(max(m, 1), dtype=torch.int64, device="cuda")
+    mmu = torch.empty(max(m, 1), dtype=torch.int64, device="cuda")
+    need = lib().u1gf_merge_workspace_bytes(m)
+    ws = _workspace(need)
+    _check(lib().u1gf_merge_copy_tables(m, _dev_ptr(F_rep.contiguous()), _dev_ptr(sig_rep.contiguous()),
+                                        _dev_ptr(first_start.contiguous()), _dev_ptr(multiplicity.contiguous()),
+                                        float(tol_F), float(tol_sig), _dev_ptr(mid), _dev_ptr(nm), _dev_ptr(mfs),
+                                        _dev_ptr(mmu), _aligned_ptr(ws), need, _stream()))
+    return dict(merged_id=mid, n_merged=nm, first_start=mfs, multiplicity=mmu)
+
+
+def pipeline_host(orbit, seed, n_starts, *, first_start=0, omega=1.7, eps=1e-13, max_sweeps=20000, check_every=1,
+                  tol_F=1e-10, tol_sig=1e-4, tol_fp=1e-8, nbins=0, out=None, copy_capacity=None):
+    """u1gf_pipeline_host: the whole hot path with host (numpy) result arrays.  `out` = host_buffers(n) reuses pinned
+    arrays; per-copy arrays hold `copy_capacity` entries (default n)."""
+    n = int(n_starts)
+    cap = n if copy_capacity is None else int(copy_capacity)
+    if out is None:
+        out = host_buffers(n, pinned=False)
+    per_copy = out.get("per_copy")
+    if per_copy is None or per_copy["lambda1"].size < cap:
+        per_copy = dict(F_rep=np.zeros(max(cap, 1)), lambda1=np.zeros(max(cap, 1)),
+                        region=np.zeros(max(cap, 1), dtype=np.uint8))
+        out["per_copy"] = per_copy
+    hist = np.zeros(nbins, dtype=np.int64) if nbins else None
+    nd, nin = np.zeros(1, dtype=np.int64), np.zeros(1, dtype=np.int64)
+    _check(lib().u1gf_pipeline_host(orbit.handle, int(seed), int(first_start), n, float(omega), float(eps), int(max_sweeps),
+                                    int(check_every), float(tol_F), float(tol_sig), float(tol_fp), int(nbins),
+                                    _np_ptr(out["F_norm"]), _np_ptr(out["sweeps"]), _np_ptr(out["status"]),
+                                    _np_ptr(out["sig"]), _np_ptr(out["copy_id"]), cap, _np_ptr(nd), _np_ptr(out["rep"]),
+                                    _np_ptr(out["multiplicity"]), _np_ptr(per_copy["F_rep"]), _np_ptr(per_copy["lambda1"]),
+                                    _np_ptr(per_copy["region"]), _np_ptr(nin), _np_ptr(hist)))
+    k = int(nd[0])
+    return dict(F_norm=out["F_norm"], sweeps=out["sweeps"], status=out["status"], sig=out["sig"], copy_id=out["copy_id"],
+                n_distinct=k, rep=out["rep"][:k], multiplicity=out["multiplicity"][:k], F_rep=per_copy["F_rep"][:k],
+                lambda1=per_copy["lambda1"][:k], region=per_copy["region"][:k], n_in_region=int(nin[0]), hist=hist)
 
 
 def _workspace(nbytes):
@@ -200,7 +369,7 @@ def relax_batch_host(orbit: Orbit, seed, n_starts, *, first_start=0, start_ids=N
     return out
 
 
-def check_fp(orbit: Orbit, g, tol_fp=1e-8):
+def check_fp(orbit: Orbit, g, tol_fp=1e-8, want_steps=False):
     """u1gf_check_fp on a device tensor g[n_cfg, V, 2] -> dict(lambda1, region, n_in_region) of device tensors."""
     import torch
     g = g.contiguous()
@@ -208,9 +377,10 @@ def check_fp(orbit: Orbit, g, tol_fp=1e-8):
     lam = torch.empty(n, dtype=torch.float64, device="cuda")
     reg = torch.empty(n, dtype=torch.uint8, device="cuda")
     cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    steps = torch.empty(n, dtype=torch.int32, device="cuda") if want_steps else None
     _check(lib().u1gf_check_fp(orbit.handle, n, _dev_ptr(g), float(tol_fp), _dev_ptr(lam), _dev_ptr(reg),
-                               _dev_ptr(cnt), _stream()))
-    return dict(lambda1=lam, region=reg, n_in_region=cnt)
+                               _dev_ptr(cnt), _dev_ptr(steps), _stream()))
+    return dict(lambda1=lam, region=reg, n_in_region=cnt, steps=steps)
 
 
 def check_fp_host(orbit: Orbit, g, tol_fp=1e-8):
@@ -284,33 +454,34 @@ def paper_count(F_norm, status, scale=1e8, workspace=None):
     return nk
 
 
+def _mcheck(rc):
+    if rc != 0:
+        raise U1gfError(rc, measure_lib().u1gf_measure_last_error().decode())
+
+
 def measure_fp64_peak(ms=200.0) -> float:
     v = C.c_double(0)
-    _check(lib().u1gf_measure_fp64_peak(float(ms), C.byref(v), _stream()))
+    _mcheck(measure_lib().u1gf_measure_fp64_peak(float(ms), C.byref(v), _stream()))
     return v.value
 
 
 def measure_fp64_rate(pattern: int, ms=200.0) -> float:
     v = C.c_double(0)
-    _check(lib().u1gf_measure_fp64_rate(int(pattern), float(ms), C.byref(v), _stream()))
+    _mcheck(measure_lib().u1gf_measure_fp64_rate(int(pattern), float(ms), C.byref(v), _stream()))
     return v.value
 
 
 def measure_smem_peak(ms=200.0) -> float:
     v = C.c_double(0)
-    _check(lib().u1gf_measure_smem_peak(float(ms), C.byref(v), _stream()))
+    _mcheck(measure_lib().u1gf_measure_smem_peak(float(ms), C.byref(v), _stream()))
     return v.value
 
 
 def measure_smem_rate(mix: int, ms=200.0) -> float:
     v = C.c_double(0)
-    _check(lib().u1gf_measure_smem_rate(int(mix), float(ms), C.byref(v), _stream()))
+    _mcheck(measure_lib().u1gf_measure_smem_rate(int(mix), float(ms), C.byref(v), _stream()))
     return v.value
 
 
 def last_launch_count() -> int:
     return int(lib().u1gf_last_launch_count())
-
-
-def last_relax_ms() -> float:
-    return float(lib().u1gf_last_relax_ms())

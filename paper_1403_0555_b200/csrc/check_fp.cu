@@ -21,6 +21,7 @@ struct FpParams {
     double* lambda1;
     uint8_t* region;
     unsigned long long* n_in;
+    int32_t* steps;   // Lanczos steps taken per configuration, or NULL
 };
 
 __device__ __forceinline__ double block_sum(double a, double (*red)[32], int& buf) {
@@ -170,7 +171,7 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
         int k = 0, next_check = 16, k_prev = 0, n_checks = 0;
         double res_prev = 0.0, last_drop = 0.0;
         bool have_drop = false;
-        bool done = false;
+        bool done = false, unconverged = false;
         while (!done) {
             // w = M v1 - beta_prev v0  (into v0), alpha = <w, v1>
             double a = 0.0;
@@ -238,6 +239,7 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
                 lam_hi = lam + 1e-9;
                 const double res = s_res;
                 if (breakdown || k == kmax || res < 1e-10) done = true;
+                unconverged = !breakdown && !(res < 1e-10) && k < V - 1;   // k = V-1: the Krylov space is the whole of 1-perp, T_k is exact
                 // next test where the residual bound, which falls geometrically, is expected to cross 1e-10
                 int step = max(4, k / 4);
                 if (n_checks > 0 && res > 0.0 && res < res_prev) {
@@ -262,11 +264,10 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
         if (tid == 0) {
             P.lambda1[cfg] = lam;
             const uint8_t reg = lam > P.tol_fp ? 1 : (fabs(lam) <= P.tol_fp ? 2 : 0);
-#ifdef U1GF_FP_DEBUG_K
-            P.region[cfg] = (uint8_t)min(k, 255);
-#else
-            P.region[cfg] = reg;
-#endif
+            // bit 2: the step cap was reached with the residual bound still above 1e-10 (R16): lambda1 is then only an
+            // upper bound of the eigenvalue and the caller should not trust a region of 1 or 2
+            P.region[cfg] = (uint8_t)(reg | (unconverged ? 4 : 0));
+            if (P.steps) P.steps[cfg] = k;
             if (reg) atomicAdd(P.n_in, 1ull);
         }
     }
@@ -306,7 +307,7 @@ int launch(const u1gf_orbit* o, const FpParams& P, cudaStream_t st) {
 using namespace u1gf;
 
 extern "C" int u1gf_check_fp(const u1gf_orbit* o, uint64_t n_cfg, const double* g, double tol_fp, double* lambda1,
-                             uint8_t* region, int64_t* n_in_region, void* cuda_stream) {
+                             uint8_t* region, int64_t* n_in_region, int32_t* lanczos_steps, void* cuda_stream) {
     t_launches = 0;
     if (!o) return fail(U1GF_EINVAL, "u1gf_check_fp: NULL orbit");
     if (!n_in_region) return fail(U1GF_EINVAL, "u1gf_check_fp: NULL n_in_region");
@@ -316,7 +317,7 @@ extern "C" int u1gf_check_fp(const u1gf_orbit* o, uint64_t n_cfg, const double* 
     U1GF_CUDA(cudaMemsetAsync(n_in_region, 0, sizeof(int64_t), st));
     if (n_cfg == 0) return U1GF_OK;
     if (!g || !lambda1 || !region) return fail(U1GF_EINVAL, "u1gf_check_fp: NULL array");
-    FpParams P{n_cfg, (const double2*)g, tol_fp, lambda1, region, (unsigned long long*)n_in_region};
+    FpParams P{n_cfg, (const double2*)g, tol_fp, lambda1, region, (unsigned long long*)n_in_region, lanczos_steps};
     switch (o->dev.d) {
         case 1: return launch<1>(o, P, st);
         case 2: return launch<2>(o, P, st);

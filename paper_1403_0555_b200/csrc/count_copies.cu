@@ -170,6 +170,15 @@ __global__ void hist_kernel(const double* __restrict__ F, const int64_t* n_disti
     }
 }
 
+__global__ void init_small_kernel(unsigned* small, unsigned n) {
+    if (threadIdx.x == 0) {
+        small[0] = 0u;
+        small[1] = 1u;
+        small[2] = 0u;
+        small[3] = n;
+    }
+}
+
 __global__ void empty_kernel(int64_t* n_distinct, int64_t* hist, int nbins) {
     if (threadIdx.x == 0 && blockIdx.x == 0) *n_distinct = 0;
     if (hist)
@@ -220,20 +229,19 @@ int u1gf_count_copies(uint64_t n_, const double* F_norm, const double* sig, cons
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const unsigned blocks = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)sms * 8);
 
-    const unsigned small_init[4] = {0u, 1u, 0u, n};
-    U1GF_CUDA(cudaMemcpyAsync(w.small, small_init, sizeof small_init, cudaMemcpyHostToDevice, st));
+    init_small_kernel<<<1, 32, 0, st>>>(w.small, n);   // on the device: no staged copy from pageable host memory
+    U1GF_CUDA(cudaGetLastError());
+    ++t_launches;
     make_keys_kernel<<<blocks, 256, 0, st>>>(n, F_norm, status, w, multiplicity, hist, nbins);
     U1GF_CUDA(cudaGetLastError());
     ++t_launches;
     size_t tb = w.cub_bytes;
     U1GF_CUDA(cub::DeviceRadixSort::SortPairs(w.cub_tmp, tb, w.keys_in, w.keys_out, w.pos_in, w.pos_out, (int)n, 0, 64, st));
-    t_launches += 8;  // CUB radix sort: histogram + onesweep passes (reported as an estimate)
     run_flags_kernel<<<blocks, 256, 0, st>>>(n, F_norm, tol_F, w);
     U1GF_CUDA(cudaGetLastError());
     ++t_launches;
     tb = w.cub_bytes;
     U1GF_CUDA(cub::DeviceScan::InclusiveSum(w.cub_tmp, tb, w.run_id, w.run_id, (int)n, st));
-    t_launches += 2;
 
     {
         int per_sm = 0;
@@ -246,7 +254,6 @@ int u1gf_count_copies(uint64_t n_, const double* F_norm, const double* sig, cons
     }
     tb = w.cub_bytes;
     U1GF_CUDA(cub::DeviceScan::ExclusiveSum(w.cub_tmp, tb, w.lead_idx, w.lead_idx, (int)n, st));
-    t_launches += 2;
     // leader flags were overwritten by their scan; assign_kernel recognises leaders by leader_of[p] == p
     assign_kernel<<<blocks, 256, 0, st>>>(n, w, copy_id, n_distinct, rep, multiplicity);
     U1GF_CUDA(cudaGetLastError());

@@ -1,6 +1,7 @@
-// peaks.cu -- roofline denominators measured on the device in use (not part of the method):
+// peaks.cu -- libu1gf_measure.so: roofline denominators measured on the device in use (not part of the method):
 // FP64 FMA issue rate (the bound of the resident relaxation kernels) and conflict-free
 // 128-bit shared-memory load bandwidth (their co-limit).
+#include "../../include/u1gf_measure.h"
 #include "u1gf_internal.h"
 
 namespace u1gf {

@@ -267,18 +267,15 @@ int launch(const u1gf_orbit* o, const Params& P, int T, cudaStream_t st, bool re
     if (per_sm < 1) return fail(U1GF_ECUDA, "generic relaxation kernel does not fit on an SM (V = %d)", o->dev.V);
     unsigned long long grid = (unsigned long long)per_sm * (unsigned long long)o->sm_count;
     if (grid > P.n_starts) grid = P.n_starts;
-    if (redo) {   // the caller zeroed the counter and brackets the whole call with its own events
+    if (redo) {   // the caller zeroed the counter
         kern<<<(unsigned)grid, T, smem, st>>>(o->dev, P);
         U1GF_CUDA(cudaGetLastError());
         ++t_launches;
         return U1GF_OK;
     }
     U1GF_CUDA(cudaMemsetAsync(P.counter, 0, sizeof(unsigned long long), st));
-    U1GF_CUDA(cudaEventRecord(t_ev0, st));
     kern<<<(unsigned)grid, T, smem, st>>>(o->dev, P);
     U1GF_CUDA(cudaGetLastError());
-    U1GF_CUDA(cudaEventRecord(t_ev1, st));
-    t_ev_valid = true;
     ++t_launches;
     return U1GF_OK;
 }

@@ -595,11 +595,8 @@ int launch_phased_k(const u1gf_orbit* o, const RelaxArgs& a, StreamParams& P, cu
     if (teams < 1) return fail(U1GF_ECUDA, "phased relaxation kernel does not fit on an SM");
     const size_t bytes = 256 + (size_t)teams * (size_t)o->dev.V * 32 * sizeof(double2);
     U1GF_CUDA(cudaMemsetAsync(a.workspace, 0, bytes, st));
-    U1GF_CUDA(cudaEventRecord(t_ev0, st));
     kern<<<(unsigned)teams, kPhasedThreads, 0, st>>>(P);
     U1GF_CUDA(cudaGetLastError());
-    U1GF_CUDA(cudaEventRecord(t_ev1, st));
-    t_ev_valid = true;
     ++t_launches;
     return U1GF_OK;
 }
@@ -618,11 +615,8 @@ int launch_k(const u1gf_orbit* o, const RelaxArgs& a, StreamParams& P, cudaStrea
     // counter and team buffers start from zero (an idle lane then reads a null field, not stale bits)
     const size_t bytes = 256 + (size_t)teams * 2 * (size_t)o->dev.V * 32 * sizeof(double2);
     U1GF_CUDA(cudaMemsetAsync(a.workspace, 0, bytes, st));
-    U1GF_CUDA(cudaEventRecord(t_ev0, st));
     kern<<<(unsigned)teams, kThreads, 0, st>>>(P);
     U1GF_CUDA(cudaGetLastError());
-    U1GF_CUDA(cudaEventRecord(t_ev1, st));
-    t_ev_valid = true;
     ++t_launches;
     return U1GF_OK;
 }

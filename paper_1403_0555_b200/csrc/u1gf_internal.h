@@ -28,10 +28,7 @@ int check_device();  // U1GF_OK or U1GF_ENODEV (cached per thread)
                                 __FILE__, __LINE__);                                           \
     } while (0)
 
-extern thread_local int t_launches;     // kernels launched by the current call
-extern thread_local cudaEvent_t t_ev0;  // events bracketing the last relaxation kernel
-extern thread_local cudaEvent_t t_ev1;
-extern thread_local bool t_ev_valid;
+extern thread_local int t_launches;     // kernels of this library launched by the current call (CUB's not counted)
 
 // ------------------------------------------------------------------------------------------------------
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11; the generator named at PAPER.md:L121, ref [59]).
@@ -132,7 +129,7 @@ struct RelaxArgs {
 size_t generic_workspace_bytes(const u1gf_orbit* o, uint64_t n);
 int generic_relax(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st);
 // redo mode: relax the starts at output positions pos[0 .. *n_dev) again (R6 fix-up of the resident kernels); `counter` is a
-// zeroed device word; no events are recorded
+// zeroed device word
 int generic_relax_list(const u1gf_orbit* o, const RelaxArgs& a, const unsigned* n_dev, const unsigned long long* pos,
                        unsigned long long* counter, cudaStream_t st);
 
@@ -143,6 +140,11 @@ size_t lanes_links_bytes(int d, const int* ext);  // extra blob bytes for the ke
 void lanes_fill_links(int d, const int* ext, const double* U_host, double2* dst_host);
 size_t lanes_workspace_bytes(const u1gf_orbit* o, uint64_t n);
 int lanes_relax(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st);
+// ensemble mode: n_orbits orbits of the shape of `o` in one launch; U_all = their lanes tables, lanes_stride
+// double2 apart; seeds_dev[n_orbits]; a.n_starts = starts per orbit; outputs at orbit * a.n_starts + k; a.start_ids unused
+size_t lanes_ens_workspace_bytes(const u1gf_orbit* o, unsigned n_orbits, uint64_t n);
+int lanes_relax_ens(const u1gf_orbit* o, const double2* U_all, unsigned long long lanes_stride,
+                    const unsigned long long* seeds_dev, unsigned n_orbits, const RelaxArgs& a, cudaStream_t st);
 
 // streamed "lane per start" kernel for the large even lattices (relax_stream.cu)
 bool stream_supported(const u1gf_orbit* o);   // every extent even

@@ -2,7 +2,7 @@
 
 `python -m paper_1403_0555_b200.microbench` prints one table (markdown) of what DESIGN.md section 7.1 quotes: the
 FP64 FMA issue rate for different operand patterns, the dependent-issue latency, the FP64 tensor-core rate, and the
-cost of the shared-memory instructions of a site update.  Everything runs in libu1gf.so (u1gf_measure_*); this module
+cost of the shared-memory instructions of a site update.  Everything runs in libu1gf_measure.so (include/u1gf_measure.h); this module
 only converts rates to cycles.  Needs a CUDA device; there is no CPU path.
 """
 from __future__ import annotations

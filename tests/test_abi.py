@@ -18,20 +18,34 @@ def binding():
     return b
 
 
-def _declared_symbols():
-    text = open(os.path.join(ROOT, "include", "u1gf.h")).read()
+def _declared_symbols(header="u1gf.h"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(u1gf_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_header_symbols_are_exported_and_bound(binding):
     declared = _declared_symbols()
-    assert len(declared) >= 20
+    assert len(declared) >= 19
     L = C.CDLL(binding.LIB_PATH)
     for name in declared:
         assert hasattr(L, name), f"{name} declared in include/u1gf.h but not exported by libu1gf.so"
     assert declared == binding.exported_symbols(), "binding._SIGNATURES must list exactly the header's symbols"
-    assert binding.lib().u1gf_abi_version() == 1
+    assert binding.lib().u1gf_abi_version() == 2
+    # the method's header carries no measurement or debug entry points; those live in include/u1gf_measure.h
+    assert not [n for n in declared if "measure" in n or n.startswith("u1gf_last_") and n != "u1gf_last_error"]
+
+
+def test_measure_header_symbols(binding):
+    declared = _declared_symbols("u1gf_measure.h")
+    assert declared == binding.measure_symbols()
+    main, meas = C.CDLL(binding.LIB_PATH), C.CDLL(binding.MEASURE_LIB_PATH)
+    for name in declared:
+        where = main if name == "u1gf_last_launch_count" else meas
+        assert hasattr(where, name), f"{name} declared in include/u1gf_measure.h but not exported"
+    for name in declared:
+        if name != "u1gf_last_launch_count":
+            assert not hasattr(main, name), f"{name}: measurement code inside the method library"
 
 
 def test_argument_validation_needs_no_device(binding):
@@ -50,7 +64,7 @@ def test_argument_validation_needs_no_device(binding):
     assert L.u1gf_create_orbit(2, p(ext), p(thn), C.byref(h)) == -1 and b"not finite" in L.u1gf_last_error()
     assert L.u1gf_create_orbit(2, None, p(th), C.byref(h)) == -1
     assert L.u1gf_relax_batch(None, 1, 0, 4, None, 1.7, 1e-13, 100, 1, None, None, None, None, None, None, 0, None) == -1
-    assert L.u1gf_check_fp(None, 1, None, 1e-8, None, None, None, None) == -1
+    assert L.u1gf_check_fp(None, 1, None, 1e-8, None, None, None, None, None) == -1
     assert L.u1gf_count_copies(1 << 31, None, None, None, 1e-10, 1e-4, None, None, None, None, None, 0, None, 0, None) == -1
     assert L.u1gf_destroy_orbit(None) == 0
     assert L.u1gf_orbit_volume(None) == 0 and L.u1gf_orbit_dim(None) == 0
