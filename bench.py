@@ -5,8 +5,13 @@ A "step" is one pass of the whole hot path (a2-a8) over one
 workload BASELINE.json's target is quoted on: config 4 = 4D 4^4, Gaussian(0.8)+gauge-transformed orbit (seed 11),
 2^22 random starts, omega 1.7, eps 1e-13:
     u1gf_relax_batch -> u1gf_count_copies -> u1gf_relax_batch(start_ids = representatives, g_canon) -> u1gf_check_fp
+(on hot orbits, where most starts are their own copy, the fields of all starts are written in the first pass instead
+and u1gf_check_fp picks the representatives by index: no second relaxation).
 `value` = relaxation site-updates/s = V * sum(sweeps) / step time (device-resident, CUDA events).
-`e2e`   = the same through the *_host C-ABI entry points (host buffers, H2D/D2H inside the timed region).
+`e2e`   = the same through u1gf_pipeline_host (host result buffers, D2H inside the timed region; the method's only
+          host input is the link field, handed to u1gf_create_orbit inside the timed region too).
+`configs` = the other BASELINE configs (1, 2, 3 as one ensemble launch, every size of 5), each timed the same way
+          with fewer repetitions, so that one driver-visible run records all five (`--no-all-configs` skips them).
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
 """
 import argparse
@@ -27,6 +32,7 @@ from paper_1403_0555_b200 import shard, synth  # noqa: E402
 METRIC = "relaxation_site_updates_per_s"
 UNIT = "site-updates/s"
 A_D = {1: 24, 2: 32, 3: 40, 4: 48}   # algorithmic FP64 instructions per site update, 8d+16
+FP64_LANES_PER_SM = 64               # B200: the DMMA probe and 148 x 64 x clock agree
 
 
 def workload(cfg_id, orbit_idx, n_override):
@@ -95,7 +101,185 @@ def oracle_leg(conf, ob, budget_s, n_first=1024):
     su = float(V) * float(r["sweeps"].sum())
     return dict(value=su / dt, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
                 sample=f"first {n} starts of the workload ({su:.3g} site-updates, {dt:.1f} s, relax+count)",
-                copies_per_s=float(((r["status"] & 1) == 0).sum()) / dt, n_distinct_in_sample=int(c["n_distinct"])), dt, su
+                copies_per_s=float(((r["status"] & 1) == 0).sum()) / dt, n_distinct_in_sample=int(c["n_distinct"]),
+                sample_starts=n), dt, su
+
+
+class Pipeline:
+    """One BASELINE workload on the device: buffers made once, `step()` = the whole hot path."""
+
+    def __init__(self, b, torch, conf, ob, first, kernel=0, nbins=10000):
+        self.b, self.torch, self.conf = b, torch, conf
+        self.ext, self.seed, self.n, self.first = ob["extents"], ob["seed"], ob["n_starts"], first
+        self.V, self.d = synth.volume(self.ext), len(self.ext)
+        self.theta = synth.make_theta(ob)
+        self.orbit = b.Orbit(self.ext, self.theta)
+        self.orbit.set_kernel(kernel)
+        self.kw = dict(omega=conf["omega"], eps=conf["eps"], max_sweeps=conf["max_sweeps"])
+        self.nbins = nbins
+        self.out = self.ws = self.cws = None
+        self.store_g = False          # decided after the first step: see step()
+        self.ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+        self.fev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+        self.state = {}
+
+    def step(self):
+        b, torch = self.b, self.torch
+        launches = 0
+        if self.store_g and (self.out is None or self.out.get("g_canon") is None):
+            self.out = None
+        self.ev[0].record()           # the relaxation kernel, on the stream it is launched on (torch's current stream)
+        self.out = b.relax_batch(self.orbit, self.seed, self.n, first_start=self.first, out=self.out, workspace=self.ws,
+                                 want_g=self.store_g, **self.kw)
+        self.ev[1].record()
+        self.ws = self.out["workspace"]
+        launches += b.last_launch_count()
+        c = b.count_copies(self.out["F_norm"], self.out["sig"], self.out["status"], nbins=self.nbins, workspace=self.cws)
+        self.cws = c["workspace"]
+        launches += b.last_launch_count()
+        nd = int(c["n_distinct"].item())                       # the only host read inside a step (8 bytes)
+        self.fev[0].record()
+        if self.store_g:
+            f = b.check_fp(self.orbit, self.out["g_canon"], index=c["rep"][:nd])
+            launches += b.last_launch_count()
+        else:
+            rr = b.relax_batch(self.orbit, self.seed, 0, start_ids=c["rep"][:nd] + self.first, want_g=True, **self.kw)
+            launches += b.last_launch_count()
+            f = b.check_fp(self.orbit, rr["g_canon"])
+            launches += b.last_launch_count()
+        self.fev[1].record()
+        # hot orbits (most starts are their own copy): write the fields of all starts in the first pass from now on,
+        # if they fit a quarter of the device memory -- no second relaxation of n_distinct ~ n representatives
+        total_mem = torch.cuda.get_device_properties(0).total_memory
+        self.store_g = nd > self.n // 4 and self.n * self.V * 16 <= total_mem // 4
+        self.state.update(n_distinct=nd, c=c, f=f, launches=launches)
+
+    def summary(self, relax_ms, fp_ms, step_ms, peak_dfma, sm_clock_mhz, sms, hbm_peak):
+        torch = self.torch
+        out, st = self.out, self.state
+        sweeps_sum = int(out["sweeps"].sum(dtype=torch.int64).item())
+        conv = int((out["status"] & 1).eq(0).sum().item())
+        su = float(self.V) * float(sweeps_sum)
+        nd = st["n_distinct"]
+        reg = st["f"]["region"]
+        exc = torch.nonzero(reg != 1).flatten()
+        exc_starts = (st["c"]["rep"][:nd][exc] + self.first).cpu().tolist()
+        fp64 = su * A_D[self.d] * 2.0 / (relax_ms * 1e-3) / 1e12
+        peak = peak_dfma * 2.0 / 1e12
+        pipe = sms * FP64_LANES_PER_SM * sm_clock_mhz * 1e6 * 2.0 / 1e12
+        name = self.orbit.kernel_name
+        roof = {"bound": "alu", "achieved": fp64, "peak": peak, "unit": "TFLOP/s", "frac": fp64 / peak,
+                "frac_of_fp64_pipe": fp64 / pipe, "fp64_pipe_peak": pipe, "traffic": None}
+        if name.startswith("stream"):
+            gbs = su * 32.0 / (relax_ms * 1e-3) / 1e9
+            roof = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                    "fp64_frac": fp64 / peak, "traffic": None}
+        roof.update(kernel=name, kernel_ms=relax_ms, kernel_share_of_step=relax_ms / step_ms)
+        return dict(workload=f"{'x'.join(map(str, self.ext))} seed {self.seed}, {self.n} starts", value=su / (step_ms * 1e-3),
+                    ms_per_step=step_ms, relax_kernel_ms=relax_ms, first_region_ms=fp_ms,
+                    first_region_path="fields of all starts kept, representatives by index" if "g_canon" in out and out["g_canon"] is not None
+                    else "representatives re-relaxed",
+                    roofline=roof, converged_copies_per_s=conv / (step_ms * 1e-3), n_distinct=nd,
+                    n_in_first_region=int(st["f"]["n_in_region"].item()),
+                    first_region_exceptions=exc_starts[:32], n_exceptions=len(exc_starts),
+                    lanczos_unconverged=int((reg & 4).ne(0).sum().item()),
+                    mean_sweeps=sweeps_sum / self.n, max_sweeps_seen=int(out["sweeps"].max().item()),
+                    gpu_launches=st["launches"]), su, conv, sweeps_sum
+
+
+def time_pipeline(p, torch, flush, steps, warmup, barrier=None):
+    for _ in range(warmup):
+        p.step()
+        flush.fill_(1)
+    if barrier:
+        barrier()
+    else:
+        torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    relax_ms, fp_ms = [], []
+    for k in range(steps):
+        ev[k][0].record()
+        p.step()
+        ev[k][1].record()
+        ev[k][1].synchronize()
+        relax_ms.append(p.ev[0].elapsed_time(p.ev[1]))
+        fp_ms.append(p.fev[0].elapsed_time(p.fev[1]))
+        flush.fill_(k & 1)
+    if barrier:
+        barrier()
+    else:
+        torch.cuda.synchronize()
+    total_ms = sum(a.elapsed_time(z) for a, z in ev)
+    return total_ms, float(np.mean(relax_ms)), float(np.mean(fp_ms))
+
+
+def ensemble_config3(b, torch, flush, steps, warmup, peak_dfma, sm_clock_mhz, sms):
+    """Config 3 (8 hot 4^3 orbits, 2^20 starts each) as ONE ensemble launch + per-orbit counting and region tests."""
+    conf = synth.CONFIGS[3]
+    obs = conf["orbits"]
+    ext, n = obs[0]["extents"], obs[0]["n_starts"]
+    V = synth.volume(ext)
+    seeds = [o["seed"] for o in obs]
+    ens = b.Ensemble(ext, np.stack([synth.make_theta(o) for o in obs]), seeds)
+    kw = dict(omega=conf["omega"], eps=conf["eps"], max_sweeps=conf["max_sweeps"])
+    st = {}
+    rev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+
+    def step():
+        rev[0].record()
+        r = b.relax_ensemble(ens, n, workspace=st.get("ws"), **kw)
+        rev[1].record()
+        launches = b.last_launch_count()
+        st["ws"] = r["workspace"]
+        c = b.count_copies_ensemble(r["F_norm"], r["sig"], r["status"], workspace=st.get("cws"))
+        launches += b.last_launch_count()
+        st["cws"] = c["workspace"]
+        nds = c["n_distinct"].cpu().tolist()
+        n_in, exc = [], []
+        for k, nd in enumerate(nds):
+            member = ens.orbit(k)
+            rr = b.relax_batch(member, seeds[k], 0, start_ids=c["rep"][k][:nd].contiguous(), want_g=True, **kw)
+            launches += b.last_launch_count()
+            f = b.check_fp(member, rr["g_canon"])
+            launches += b.last_launch_count()
+            st.setdefault("f", {})[k] = (f, c["rep"][k][:nd])
+        st.update(r=r, nds=nds, launches=launches)
+
+    for _ in range(warmup):
+        step()
+        flush.fill_(1)
+    torch.cuda.synchronize()
+    ms, rms = [], []
+    for k in range(steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        step()
+        e1.record()
+        e1.synchronize()
+        ms.append(e0.elapsed_time(e1))
+        rms.append(rev[0].elapsed_time(rev[1]))
+        flush.fill_(k & 1)
+    r = st["r"]
+    sweeps = r["sweeps"].sum(dim=1, dtype=torch.int64).cpu().tolist()
+    su = float(V) * float(sum(sweeps))
+    step_ms, relax_ms = float(np.mean(ms)), float(np.mean(rms))
+    n_in = [int(st["f"][k][0]["n_in_region"].item()) for k in range(len(seeds))]
+    exc = {int(seeds[k]): st["f"][k][1][torch.nonzero(st["f"][k][0]["region"] != 1).flatten()].cpu().tolist() for k in range(len(seeds))}
+    fp64 = su * A_D[3] * 2.0 / (relax_ms * 1e-3) / 1e12
+    peak = peak_dfma * 2.0 / 1e12
+    pipe = sms * FP64_LANES_PER_SM * sm_clock_mhz * 1e6 * 2.0 / 1e12
+    out = dict(workload=f"8 orbits 4x4x4 seeds 3..10, {n} starts each, ONE u1gf_relax_ensemble launch", value=su / (step_ms * 1e-3),
+               ms_per_step=step_ms, relax_kernel_ms=relax_ms,
+               roofline={"bound": "alu", "achieved": fp64, "peak": peak, "unit": "TFLOP/s", "frac": fp64 / peak,
+                         "frac_of_fp64_pipe": fp64 / pipe, "kernel": "lanes_4x4x4_blk4x2x2 (ensemble mode)", "kernel_ms": relax_ms,
+                         "kernel_share_of_step": relax_ms / step_ms, "traffic": None},
+               converged_copies_per_s=float((r["status"] & 1).eq(0).sum().item()) / (step_ms * 1e-3),
+               n_distinct_per_orbit=st["nds"], n_in_first_region_per_orbit=n_in,
+               first_region_exceptions={k: v for k, v in exc.items() if v},
+               mean_sweeps_per_orbit=[s / n for s in sweeps], max_sweeps_per_orbit=r["sweeps"].max(dim=1).values.cpu().tolist(),
+               gpu_launches=st["launches"])
+    ens.close()
+    return out
 
 
 def main():
@@ -110,6 +294,7 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 force the generic kernel")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-all-configs", action="store_true", help="skip the `configs` section (BASELINE configs 1-3, 5)")
     args = ap.parse_args()
 
     ri = shard.rank_info_from_env()
@@ -133,8 +318,13 @@ def main():
             vals.append(su); dts.append(dt)
         v = sum(vals) / sum(dts)
         last["value"] = v
+        # a step of this arm is a bounded sample of the workload; ms_per_step is the time a full step (all n starts)
+        # takes at the measured rate, ms_per_sample the time actually spent per repetition
+        full_ms = 1e3 * (sum(dts) / len(dts)) * n / last["sample_starts"]
         print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": 0,
-                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(dts) / len(dts),
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": full_ms,
+                          "ms_per_sample": 1e3 * sum(dts) / len(dts),
+                          "ms_per_step_note": "extrapolated from the sample to all starts of the workload at the measured rate",
                           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
                           "data": "synthetic", "config": config, "cpu_baseline": last,
                           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
@@ -149,34 +339,9 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     b.lib()
-    th = synth.make_theta(ob)
-    orbit = b.Orbit(ext, th)
-    orbit.set_kernel(args.kernel)
     first, _ = shard.weak_start_range(rank, world, n)   # disjoint start ranges of the same orbit, no data-path collective
-    kw = dict(omega=conf["omega"], eps=conf["eps"], max_sweeps=conf["max_sweeps"])
-    nbins = 10000
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    out = ws = cws = None
-    state = {}
-
-    def step():
-        nonlocal out, ws, cws
-        launches = 0
-        out = b.relax_batch(orbit, seed, n, first_start=first, out=out, workspace=ws, **kw)
-        ws = out["workspace"]
-        launches += b.last_launch_count()
-        state["relax_ms"] = None
-        c = b.count_copies(out["F_norm"], out["sig"], out["status"], nbins=nbins, workspace=cws)
-        cws = c["workspace"]
-        launches += b.last_launch_count()
-        nd = int(c["n_distinct"].item())                       # the only host read inside a step (8 bytes)
-        state["relax_ms"] = b.last_relax_ms()
-        rep_ids = c["rep"][:nd] + first
-        rr = b.relax_batch(orbit, seed, 0, start_ids=rep_ids, want_g=True, **kw)
-        launches += b.last_launch_count()
-        f = b.check_fp(orbit, rr["g_canon"])
-        launches += b.last_launch_count()
-        state.update(n_distinct=nd, c=c, f=f, launches=launches)
+    sms = torch.cuda.get_device_properties(local).multi_processor_count
 
     def barrier():
         torch.cuda.synchronize()
@@ -184,53 +349,53 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
+    pipe = Pipeline(b, torch, conf, ob, first, kernel=args.kernel)
+    sampler = ClockSampler(local)
     for _ in range(args.warmup):
-        step()
+        pipe.step()
         flush.fill_(1)
     barrier()
-    sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    relax_ms = []
-    for k in range(args.steps):
-        ev[k][0].record()
-        step()
-        ev[k][1].record()
-        relax_ms.append(state["relax_ms"])
-        flush.fill_(k & 1)
-    barrier()
+    total_ms, relax_ms, fp_ms = time_pipeline(pipe, torch, flush, args.steps, 0, barrier)
     clocks = sampler.stop() if rank == 0 else None
-    total_ms = sum(a.elapsed_time(z) for a, z in ev)
-    sweeps_sum = int(out["sweeps"].sum(dtype=torch.int64).item())
-    conv = int((out["status"] & 1).eq(0).sum().item())
-    total_ms, (sweeps_sum, conv) = shard.aggregate(total_ms, [sweeps_sum, conv], dist, device="cuda")
+    sm_clock = (clocks or {}).get("sm_mhz") or 1965.0
+
+    # roofline denominators: the in-run DFMA microbenchmark (libu1gf_measure.so) and the driver's HBM figure
+    peak_dfma = b.measure_fp64_peak(300.0)
+    hbm_peak, hbm_how = 6650.0, "fallback of B200_PROFILING.md"
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            hbm_peak, hbm_how = float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json"
+    except (OSError, KeyError, ValueError):
+        pass
+    main_sum, su_rank, conv, sweeps_sum = pipe.summary(relax_ms, fp_ms, total_ms / args.steps, peak_dfma, sm_clock, sms, hbm_peak)
+    total_ms, (sweeps_all, conv_all) = shard.aggregate(total_ms, [sweeps_sum, conv], dist, device="cuda")
     ms_per_step = total_ms / args.steps
-    site_updates = float(V) * float(sweeps_sum)              # per step, all ranks
+    site_updates = float(V) * float(sweeps_all)              # per step, all ranks
     value = site_updates / (ms_per_step * 1e-3)
 
-    # e2e: the same step through the host-buffer C-ABI entry points (H2D / D2H and allocation inside)
+    # e2e: the whole path through u1gf_pipeline_host: link angles in (u1gf_create_orbit), host result arrays out
     e2e = None
     if not args.no_e2e:
         hb = b.host_buffers(n)   # pinned result arrays, made once: the timed region holds copies, not page faults
+        th = pipe.theta
+        kw = pipe.kw
 
         def host_step():
             orb = b.Orbit(ext, th)
             orb.set_kernel(args.kernel)
-            r = b.relax_batch_host(orb, seed, n, first_start=first, out=hb, **kw)
-            c = b.count_copies_host(r["F_norm"], r["sig"], r["status"], nbins=nbins, out=hb)
-            rr = b.relax_batch_host(orb, seed, 0, start_ids=(c["rep"] + first).astype(np.uint64), want_g=True, **kw)
-            f = b.check_fp_host(orb, rr["g_canon"])
-            nd = c["n_distinct"]
-            h2d = th.nbytes + n * 41 + nd * 8 + nd * V * 16
-            d2h = n * 45 + n * 4 + 8 + 2 * nd * 8 + nbins * 8 + nd * (45 + V * 16) + nd * 9 + 8
+            p = b.pipeline_host(orb, seed, n, first_start=first, nbins=10000, out=hb, **kw)
+            nd = p["n_distinct"]
+            h2d = th.nbytes
+            d2h = n * (8 + 4 + 1 + 32 + 4) + 8 + nd * (8 + 8 + 8 + 8 + 1) + 10000 * 8 + 8 * (1 + (nd + 0) // max(1, (1 << 30) // (V * 16)))
             orb.close()
-            return float(V) * float(r["sweeps"].sum()), h2d, d2h
+            return float(V) * float(p["sweeps"].sum(dtype=np.int64)), h2d, d2h
         host_step()
         barrier()
         t0 = time.perf_counter()
         su_e = 0.0
-        reps = max(1, min(args.steps, 2))
+        reps = max(1, args.steps)
         for _ in range(reps):
             su, h2d, d2h = host_step()
             su_e += su
@@ -240,55 +405,56 @@ def main():
         if dist:
             dist.all_reduce(te, op=dist.ReduceOp.MAX)
         e2e = {"value": su_e * world / float(te[0]), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-               "d2h_bytes_per_step": int(d2h), "timing": "wall clock around the synchronous *_host calls, max over ranks"}
+               "d2h_bytes_per_step": int(d2h), "repetitions": reps, "call": "u1gf_create_orbit + u1gf_pipeline_host",
+               "timing": "wall clock around the synchronous calls, max over ranks"}
+        b.lib().u1gf_release_host_scratch()
 
     if rank != 0:
         if dist:
             dist.destroy_process_group()
         return 0
 
-    # roofline of the dominant kernel (the relaxation kernel): FP64 ALU bound
-    peak_dfma = b.measure_fp64_peak(300.0)
     rate_rrr = b.measure_fp64_rate(1, 100.0)   # DFMA with three distinct register operands
     rate_mac = b.measure_fp64_rate(2, 100.0)   # the complex multiply-accumulate pattern of w_i
-    k_ms = float(np.mean([m for m in relax_ms if m and m > 0])) if any(relax_ms) else None
-    per_rank_su = site_updates / world
-    achieved = per_rank_su * A_D[d] * 2.0 / (k_ms * 1e-3) / 1e12 if k_ms else None
-    peak = peak_dfma * 2.0 / 1e12
-    roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak if achieved else None, "traffic": None,
-                "dfma_rate_3_register_operands": rate_rrr * 2.0 / 1e12, "dfma_rate_complex_mac": rate_mac * 2.0 / 1e12,
-                "kernel": orbit.kernel_name, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_per_step if k_ms else None,
-                "note": ("achieved = site-updates x (8d+16 = %d algorithmic FP64 instructions) x 2 flop / kernel time; "
-                         "peak = 2 x DFMA/s of the in-run u1gf_measure_fp64_peak microbenchmark (kernel timed alone; constant "
-                         "multiplicands); dfma_rate_* = the same unit for DFMA streams with register multiplicands, "
-                         "which the register file limits to 3/4 of peak (DESIGN.md section 7.1)") % A_D[d]}
-    if orbit.kernel_name.startswith("stream"):
-        # the streamed kernel (large lattices) is bound by memory traffic: algorithmic bytes = one read and one write of
-        # g per site update (32 B); peak = the driver's measured HBM copy bandwidth
-        hbm_peak, how = 6650.0, "fallback of B200_PROFILING.md"
-        try:
-            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-                hbm_peak, how = float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json"
-        except (OSError, KeyError, ValueError):
-            pass
-        gbs = per_rank_su * 32.0 / (k_ms * 1e-3) / 1e9 if k_ms else None
-        roofline = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
-                    "frac": gbs / hbm_peak if gbs else None, "traffic": None, "peak_source": how,
-                    "fp64_frac": roofline["frac"], "kernel": orbit.kernel_name, "kernel_ms": k_ms,
-                    "kernel_share_of_step": k_ms / ms_per_step if k_ms else None,
-                    "note": "achieved = site-updates x 32 algorithmic bytes / kernel time; fp64_frac = the same launch "
-                            "against the measured FP64 peak (A_d algorithmic instructions per site update)"}
+    rate_dmma = b.measure_fp64_rate(6, 100.0)  # the FP64 pipe through DMMA: 64 lanes x SMs x clock
+    roofline = main_sum["roofline"]
+    roofline.update({"peak_source": "in-run u1gf_measure_fp64_peak (DFMA stream, constant multiplicands), kernel timed alone",
+                     "dmma_rate": rate_dmma * 2.0 / 1e12, "frac_of_dmma_rate": roofline.get("achieved", 0.0) / (rate_dmma * 2.0 / 1e12)
+                     if roofline["bound"] == "alu" else None,
+                     "dfma_rate_3_register_operands": rate_rrr * 2.0 / 1e12, "dfma_rate_complex_mac": rate_mac * 2.0 / 1e12,
+                     "hbm_peak_source": hbm_how,
+                     "note": ("achieved = site-updates x (8d+16 = %d algorithmic FP64 instructions) x 2 flop / kernel time "
+                              "(CUDA events on the launching stream around u1gf_relax_batch); frac = against the DFMA "
+                              "microbenchmark, frac_of_fp64_pipe / frac_of_dmma_rate = against 64 lanes x SMs x clock, which "
+                              "only DMMA reaches (DESIGN.md section 7.1)") % A_D[d]})
+
+    configs = None
+    if not args.no_all_configs and world == 1 and not args.starts:
+        configs = {}
+        csteps, cwarm = 2, 1
+        for cid, oi in [(1, 0), (2, 0)] + [(5, k) for k in range(5)]:
+            c2, o2 = workload(cid, oi, 0)
+            p2 = Pipeline(b, torch, c2, o2, 0)
+            t_ms, r_ms, f_ms = time_pipeline(p2, torch, flush, csteps, cwarm + (1 if cid == 5 and oi >= 2 else 0))
+            s2, _, _, _ = p2.summary(r_ms, f_ms, t_ms / csteps, peak_dfma, sm_clock, sms, hbm_peak)
+            s2.update(steps=csteps, warmup=cwarm)
+            configs[f"cfg{cid}_{'x'.join(map(str, o2['extents']))}"] = s2
+            del p2
+            torch.cuda.empty_cache()
+        configs["cfg3_ensemble"] = ensemble_config3(b, torch, flush, csteps, cwarm, peak_dfma, sm_clock, sms)
+
     cpu = None
     if not args.no_cpu_baseline:
         cpu, _, _ = oracle_leg(conf, ob, 10.0)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": config, "clocks": clocks, "e2e": e2e, "gpu_launches": state["launches"],
+            "data": "synthetic", "config": config, "clocks": clocks, "e2e": e2e, "gpu_launches": main_sum["gpu_launches"],
+            "gpu_launches_note": "kernels of libu1gf.so per step, counted by the library; CUB's sort/scan launches inside u1gf_count_copies are extra",
             "roofline": roofline, "cpu_baseline": cpu,
-            "converged_copies_per_s": conv / (ms_per_step * 1e-3), "n_distinct": state["n_distinct"],
-            "n_in_first_region": int(state["f"]["n_in_region"].item()), "mean_sweeps": sweeps_sum / (n * world)}
+            "converged_copies_per_s": conv_all / (ms_per_step * 1e-3), "n_distinct": main_sum["n_distinct"],
+            "n_in_first_region": main_sum["n_in_first_region"], "first_region_exceptions": main_sum["first_region_exceptions"],
+            "mean_sweeps": sweeps_all / (n * world), "max_sweeps_seen": main_sum["max_sweeps_seen"], "configs": configs}
     print(json.dumps(line))
     if dist:
         dist.destroy_process_group()

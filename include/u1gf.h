@@ -111,7 +111,10 @@ const char* u1gf_kernel_name(const u1gf_orbit* o);
  * (M v)_i = sum_mu [c_{i,mu}(v_i - v_{i+mu}) + c_{i-mu,mu}(v_i - v_{i-mu})]; lambda_1 = smallest eigenvalue of M on
  * the orthogonal complement of the constant vector (the global gauge zero mode), computed by a
  * batched matrix-free Lanczos iteration (one CTA per configuration).
- *   g           dev [n_cfg*V*2]
+ *   g           dev [.*V*2] configurations
+ *   cfg_index   dev [n_cfg] int64 or NULL: configuration k is g[cfg_index[k]] (NULL: g[k]).  With it the fields of ALL
+ *               starts, written once by u1gf_relax_batch(g_canon), serve the representatives without a gather or a
+ *               second relaxation (the choice when most starts are their own copy: hot 4^4 and larger)
  *   tol_fp      region bits 0-1 = 1 if lambda_1 > tol_fp (inside), 2 if |lambda_1| <= tol_fp (marginal, "semi"definite),
  *               0 if lambda_1 < -tol_fp (outside); region bit 2 (value 4) is set when the iteration reached its cap of
  *               min(V-1, 512) steps with the Ritz residual bound still above 1e-10 (R16): lambda1 is then only an upper
@@ -121,8 +124,8 @@ const char* u1gf_kernel_name(const u1gf_orbit* o);
  * A converged relaxation can stop at a saddle it is still leaving (the stop rule tests the gradient only):
  * such copies come out with region 0 and are genuine -- DESIGN.md section 3, R17.
  * ------------------------------------------------------------------------------------------------------- */
-int u1gf_check_fp(const u1gf_orbit* o, uint64_t n_cfg, const double* g, double tol_fp, double* lambda1,
-                  uint8_t* region, int64_t* n_in_region, int32_t* lanczos_steps, void* cuda_stream);
+int u1gf_check_fp(const u1gf_orbit* o, uint64_t n_cfg, const double* g, const int64_t* cfg_index, double tol_fp,
+                  double* lambda1, uint8_t* region, int64_t* n_in_region, int32_t* lanczos_steps, void* cuda_stream);
 int u1gf_check_fp_host(const u1gf_orbit* o, uint64_t n_cfg, const double* g_host, double tol_fp,
                        double* lambda1_host, uint8_t* region_host, int64_t* n_in_region_host);
 

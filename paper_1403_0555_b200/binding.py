@@ -29,7 +29,7 @@ _SIGNATURES = {
                                         C.c_int32, C.c_int32, _p, _p, _p, _p, _p]),
     "u1gf_set_kernel": (C.c_int, [_p, C.c_int32]),
     "u1gf_kernel_name": (C.c_char_p, [_p]),
-    "u1gf_check_fp": (C.c_int, [_p, C.c_uint64, _p, C.c_double, _p, _p, _p, _p, _p]),
+    "u1gf_check_fp": (C.c_int, [_p, C.c_uint64, _p, _p, C.c_double, _p, _p, _p, _p, _p]),
     "u1gf_check_fp_host": (C.c_int, [_p, C.c_uint64, _p, C.c_double, _p, _p, _p]),
     "u1gf_count_workspace_bytes": (C.c_size_t, [C.c_uint64]),
     "u1gf_count_copies": (C.c_int, [C.c_uint64, _p, _p, _p, C.c_double, C.c_double, _p, _p, _p, _p, _p, C.c_int32,
@@ -369,16 +369,20 @@ def relax_batch_host(orbit: Orbit, seed, n_starts, *, first_start=0, start_ids=N
     return out
 
 
-def check_fp(orbit: Orbit, g, tol_fp=1e-8, want_steps=False):
-    """u1gf_check_fp on a device tensor g[n_cfg, V, 2] -> dict(lambda1, region, n_in_region) of device tensors."""
+def check_fp(orbit: Orbit, g, tol_fp=1e-8, want_steps=False, index=None):
+    """u1gf_check_fp on a device tensor g[., V, 2] -> dict(lambda1, region, n_in_region) of device tensors.  `index`
+    (device int64 tensor) selects the configurations g[index[k]]; without it all of g is tested."""
     import torch
     g = g.contiguous()
     n = int(g.shape[0]) if g.numel() else 0
+    if index is not None:
+        index = index.contiguous()
+        n = int(index.numel())
     lam = torch.empty(n, dtype=torch.float64, device="cuda")
     reg = torch.empty(n, dtype=torch.uint8, device="cuda")
     cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
     steps = torch.empty(n, dtype=torch.int32, device="cuda") if want_steps else None
-    _check(lib().u1gf_check_fp(orbit.handle, n, _dev_ptr(g), float(tol_fp), _dev_ptr(lam), _dev_ptr(reg),
+    _check(lib().u1gf_check_fp(orbit.handle, n, _dev_ptr(g), _dev_ptr(index), float(tol_fp), _dev_ptr(lam), _dev_ptr(reg),
                                _dev_ptr(cnt), _dev_ptr(steps), _stream()))
     return dict(lambda1=lam, region=reg, n_in_region=cnt, steps=steps)
 

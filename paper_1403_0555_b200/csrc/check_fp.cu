@@ -22,6 +22,7 @@ struct FpParams {
     uint8_t* region;
     unsigned long long* n_in;
     int32_t* steps;   // Lanczos steps taken per configuration, or NULL
+    const int64_t* index;   // configuration k is g[index[k]] (NULL: g[k])
 };
 
 __device__ __forceinline__ double block_sum(double a, double (*red)[32], int& buf) {
@@ -134,7 +135,7 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
     const int kmax = kcap;
 
     for (unsigned long long cfg = blockIdx.x; cfg < P.n_cfg; cfg += gridDim.x) {
-        const double2* g = P.g + cfg * (unsigned long long)V;
+        const double2* g = P.g + (P.index ? (unsigned long long)P.index[cfg] : cfg) * (unsigned long long)V;
         __syncthreads();
         for (int l = tid; l < V * DIM; l += T) {
             const int i = l / DIM, mu = l - i * DIM;
@@ -306,8 +307,9 @@ int launch(const u1gf_orbit* o, const FpParams& P, cudaStream_t st) {
 
 using namespace u1gf;
 
-extern "C" int u1gf_check_fp(const u1gf_orbit* o, uint64_t n_cfg, const double* g, double tol_fp, double* lambda1,
-                             uint8_t* region, int64_t* n_in_region, int32_t* lanczos_steps, void* cuda_stream) {
+extern "C" int u1gf_check_fp(const u1gf_orbit* o, uint64_t n_cfg, const double* g, const int64_t* cfg_index,
+                             double tol_fp, double* lambda1, uint8_t* region, int64_t* n_in_region,
+                             int32_t* lanczos_steps, void* cuda_stream) {
     t_launches = 0;
     if (!o) return fail(U1GF_EINVAL, "u1gf_check_fp: NULL orbit");
     if (!n_in_region) return fail(U1GF_EINVAL, "u1gf_check_fp: NULL n_in_region");
@@ -317,7 +319,7 @@ extern "C" int u1gf_check_fp(const u1gf_orbit* o, uint64_t n_cfg, const double* 
     U1GF_CUDA(cudaMemsetAsync(n_in_region, 0, sizeof(int64_t), st));
     if (n_cfg == 0) return U1GF_OK;
     if (!g || !lambda1 || !region) return fail(U1GF_EINVAL, "u1gf_check_fp: NULL array");
-    FpParams P{n_cfg, (const double2*)g, tol_fp, lambda1, region, (unsigned long long*)n_in_region, lanczos_steps};
+    FpParams P{n_cfg, (const double2*)g, tol_fp, lambda1, region, (unsigned long long*)n_in_region, lanczos_steps, cfg_index};
     switch (o->dev.d) {
         case 1: return launch<1>(o, P, st);
         case 2: return launch<2>(o, P, st);

@@ -110,8 +110,8 @@ int u1gf_check_fp_host(const u1gf_orbit* o, uint64_t n_cfg, const double* g_host
         return fail(U1GF_ENOMEM, "u1gf_check_fp_host: device allocation failed");
     g.take(n * V * 16); lam.take(n * 8); reg.take(n); cnt.take(8);
     U1GF_CUDA(cudaMemcpy(g.p, g_host, n * V * 16, cudaMemcpyHostToDevice));
-    int rc = u1gf_check_fp(o, n_cfg, (const double*)g.p, tol_fp, (double*)lam.p, (uint8_t*)reg.p, (int64_t*)cnt.p,
-                           nullptr, nullptr);
+    int rc = u1gf_check_fp(o, n_cfg, (const double*)g.p, nullptr, tol_fp, (double*)lam.p, (uint8_t*)reg.p,
+                           (int64_t*)cnt.p, nullptr, nullptr);
     if (rc) return rc;
     if (lambda1_host) U1GF_CUDA(cudaMemcpy(lambda1_host, lam.p, n * 8, cudaMemcpyDeviceToHost));
     if (region_host) U1GF_CUDA(cudaMemcpy(region_host, reg.p, n, cudaMemcpyDeviceToHost));
@@ -228,8 +228,8 @@ int u1gf_pipeline_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_start,
                               (int32_t*)sw2.p, (uint8_t*)st2.p, (double*)sg2.p, (double*)gc.p, wsb.p, ws, nullptr);
         if (rc) return rc;
         launches += t_launches;
-        rc = u1gf_check_fp(o, m, (const double*)gc.p, tol_fp, (double*)lam.p + a, (uint8_t*)reg.p + a, nin_dev, nullptr,
-                           nullptr);
+        rc = u1gf_check_fp(o, m, (const double*)gc.p, nullptr, tol_fp, (double*)lam.p + a, (uint8_t*)reg.p + a, nin_dev,
+                           nullptr, nullptr);
         if (rc) return rc;
         launches += t_launches;
         int64_t part = 0;

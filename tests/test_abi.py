@@ -64,7 +64,7 @@ def test_argument_validation_needs_no_device(binding):
     assert L.u1gf_create_orbit(2, p(ext), p(thn), C.byref(h)) == -1 and b"not finite" in L.u1gf_last_error()
     assert L.u1gf_create_orbit(2, None, p(th), C.byref(h)) == -1
     assert L.u1gf_relax_batch(None, 1, 0, 4, None, 1.7, 1e-13, 100, 1, None, None, None, None, None, None, 0, None) == -1
-    assert L.u1gf_check_fp(None, 1, None, 1e-8, None, None, None, None, None) == -1
+    assert L.u1gf_check_fp(None, 1, None, None, 1e-8, None, None, None, None, None) == -1
     assert L.u1gf_count_copies(1 << 31, None, None, None, 1e-10, 1e-4, None, None, None, None, None, 0, None, 0, None) == -1
     assert L.u1gf_destroy_orbit(None) == 0
     assert L.u1gf_orbit_volume(None) == 0 and L.u1gf_orbit_dim(None) == 0

@@ -44,7 +44,21 @@ def _worker(rank, world, port, q):
         r = oracle.relax(EXT, th, SEED, n, first_start=first)
         ms = 10.0 + 5.0 * rank                                   # pretend rank 1 was the slow one
         t, (sw, conv) = shard.aggregate(ms, [int(r["sweeps"].sum()), int(((r["status"] & 1) == 0).sum())], dist)
-        q.put((rank, first, n, r["sweeps"].copy(), r["F_norm"].copy(), t, sw, conv))
+        # copy tables of the ranks -> one table of the job.  The identification of copies across ranks is
+        # u1gf_merge_copy_tables on the GPU; here (CPU, test) the oracle's count_copies on the gathered entries, ordered by
+        # first start, stands in for it -- the host logic under test is the gather, the offsets and the id mapping.
+        c = oracle.count_copies(r["F_norm"], r["sig"], r["status"])
+        rep = c["rep"]
+        F, S, fs, mu, offs = shard.gather_copy_tables(torch.as_tensor(r["F_norm"][rep]), torch.as_tensor(r["sig"][rep]),
+                                                      torch.as_tensor(rep + first), torch.as_tensor(c["multiplicity"]), dist)
+        order = np.argsort(fs.numpy(), kind="stable")
+        mc = oracle.count_copies(F.numpy()[order], S.numpy()[order], np.zeros(order.size, dtype=np.uint8))
+        merged_id = np.empty(order.size, dtype=np.int64)
+        merged_id[order] = mc["copy_id"]
+        gid = shard.global_copy_ids(torch.as_tensor(c["copy_id"]), torch.as_tensor(merged_id), offs[rank]).numpy()
+        merged_mult = np.bincount(merged_id, weights=mu.numpy().astype(np.float64), minlength=mc["n_distinct"]).astype(np.int64)
+        q.put((rank, first, n, r["sweeps"].copy(), r["F_norm"].copy(), t, sw, conv, gid, mc["n_distinct"], merged_mult,
+               r["sig"].copy(), r["status"].copy()))
     finally:
         dist.destroy_process_group()
 
@@ -88,7 +102,7 @@ def test_two_ranks_gloo(oracle):
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    (r0, f0, n0, sw0, F0, t0, s0, c0), (r1, f1, n1, sw1, F1, t1, s1, c1) = res
+    (r0, f0, n0, sw0, F0, t0, s0, c0, g0, nm0, mm0, sg0, st0), (r1, f1, n1, sw1, F1, t1, s1, c1, g1, nm1, mm1, sg1, st1) = res
     assert (f0, n0, f1, n1) == (0, N_PER_RANK, N_PER_RANK, N_PER_RANK)
     # the same job in one process
     th = synth.uniform_links(EXT, SEED)
@@ -99,3 +113,8 @@ def test_two_ranks_gloo(oracle):
     assert t0 == t1 == 15.0
     assert s0 == s1 == float(whole["sweeps"].sum())
     assert c0 == c1 == float(((whole["status"] & 1) == 0).sum())
+    # merged copy tables: every start gets the id one process over all starts gives it; multiplicities add up
+    oc = oracle.count_copies(whole["F_norm"], whole["sig"], whole["status"])
+    assert nm0 == nm1 == oc["n_distinct"]
+    assert (np.concatenate([g0, g1]) == oc["copy_id"]).all()
+    assert (mm0 == oc["multiplicity"]).all() and (mm1 == oc["multiplicity"]).all()
