@@ -117,52 +117,106 @@ __device__ double last_component(const double* alpha, const double* beta, const 
     return fabs(last) * rsqrt(norm2);
 }
 
-template <int DIM>
-__global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const FpParams P) {
+// Sum of two values over the CTA, same result in every thread, fixed tree (see block_sum).
+__device__ __forceinline__ void block_sum2(double& a, double& b, double (*red2)[32][2], int& buf) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_down_sync(0xffffffffu, a, o);
+        b += __shfl_down_sync(0xffffffffu, b, o);
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0) {
+        red2[buf][warp][0] = a;
+        red2[buf][warp][1] = b;
+    }
+    __syncthreads();
+    double sa = 0.0, sb = 0.0;
+    for (int w = 0; w < nw; ++w) {
+        sa += red2[buf][w][0];
+        sb += red2[buf][w][1];
+    }
+    a = sa;
+    b = sb;
+    buf ^= 1;
+}
+
+// One CTA per configuration, every thread owns up to SPT sites (i = tid, tid + T, ...).  The neighbour indices of a
+// thread's sites are the same for every configuration and every step: they are read once into registers (16-bit,
+// V <= 8192) instead of 2 DIM index loads per site and mat-vec.  Per Lanczos step: the mat-vec with <w, v1> (one
+// reduction), w -= alpha v1 with the mean of w and its norm without the mean, sum w^2 - V mean^2, in ONE reduction, then
+// the scaled vector -- three barriers per step.
+template <int DIM, int SPT, int MAXT>
+__global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) lanczos_kernel(const OrbitDev D, const FpParams P) {
     extern __shared__ double sm[];
     const int V = D.V, tid = threadIdx.x, T = blockDim.x;
-    double* c = sm;                 // [V*DIM]
+    double* c = sm;                 // [DIM][V]
     double* va = c + (size_t)V * DIM;  // [V]
     double* vb = va + V;            // [V]
     __shared__ double red[2][32];
+    __shared__ double red2[2][32][2];
     const int kcap = min(V - 1, kMaxK);
     double* alpha = vb + V;   // Lanczos coefficients [4][kcap], behind the vectors in dynamic shared memory
     double* beta = alpha + kcap;
     double* beta2 = beta + kcap;
     double* ibeta = beta2 + kcap;
     __shared__ double s_lam, s_res;
-    int buf = 0;
+    int buf = 0, buf2 = 0;
     const int kmax = kcap;
+
+    unsigned short nf[SPT][DIM], nb[SPT][DIM];
+#pragma unroll
+    for (int s = 0; s < SPT; ++s) {
+        const int i = tid + s * T;
+#pragma unroll
+        for (int mu = 0; mu < DIM; ++mu) {
+            nf[s][mu] = i < V ? (unsigned short)__ldg(D.fwd + i * DIM + mu) : (unsigned short)0;
+            nb[s][mu] = i < V ? (unsigned short)__ldg(D.bwd + i * DIM + mu) : (unsigned short)0;
+        }
+    }
 
     for (unsigned long long cfg = blockIdx.x; cfg < P.n_cfg; cfg += gridDim.x) {
         const double2* g = P.g + (P.index ? (unsigned long long)P.index[cfg] : cfg) * (unsigned long long)V;
         __syncthreads();
-        for (int l = tid; l < V * DIM; l += T) {   // weights stored [mu][V]: consecutive lanes, consecutive banks
-            const int i = l / DIM, mu = l - i * DIM;
-            const double2 gi = g[i], gj = g[__ldg(D.fwd + l)], u = __ldg(D.U + l);
-            const double ar = gi.x * u.x - gi.y * u.y, ai = gi.x * u.y + gi.y * u.x;
-            c[mu * V + i] = ar * gj.x + ai * gj.y;
-        }
-        // start vector: fixed pseudo-random signs/values, constant mode removed, normalised
+        // weights c_{i,mu} = Re(g_i U_{i,mu} conj g_{i+mu}), stored [mu][V]: consecutive lanes, consecutive banks
         double s1 = 0.0;
-        for (int i = tid; i < V; i += T) {
-            const u32x4 r = philox((uint32_t)i, 0u, 0u, 5u, 0x52u, 0u);
-            const double x = unit_interval_pm1(r.x, r.y);
-            va[i] = x;
-            s1 += x;
+#pragma unroll
+        for (int s = 0; s < SPT; ++s) {
+            const int i = tid + s * T;
+            if (i < V) {
+                const double2 gi = g[i];
+#pragma unroll
+                for (int mu = 0; mu < DIM; ++mu) {
+                    const double2 gj = g[nf[s][mu]], u = __ldg(D.U + i * DIM + mu);
+                    const double ar = gi.x * u.x - gi.y * u.y, ai = gi.x * u.y + gi.y * u.x;
+                    c[mu * V + i] = ar * gj.x + ai * gj.y;
+                }
+                // start vector: fixed pseudo-random values, constant mode removed, normalised (R16)
+                const u32x4 r = philox((uint32_t)i, 0u, 0u, 5u, 0x52u, 0u);
+                const double x = unit_interval_pm1(r.x, r.y);
+                va[i] = x;
+                s1 += x;
+            }
         }
         s1 = block_sum(s1, red, buf);
         const double mean0 = s1 / (double)V;
         double s2 = 0.0;
-        for (int i = tid; i < V; i += T) {
-            const double x = va[i] - mean0;
-            va[i] = x;
-            s2 = fma(x, x, s2);
-            vb[i] = 0.0;
+#pragma unroll
+        for (int s = 0; s < SPT; ++s) {
+            const int i = tid + s * T;
+            if (i < V) {
+                const double x = va[i] - mean0;
+                va[i] = x;
+                s2 = fma(x, x, s2);
+                vb[i] = 0.0;
+            }
         }
         s2 = block_sum(s2, red, buf);
         const double inv0 = rsqrt(s2);
-        for (int i = tid; i < V; i += T) va[i] *= inv0;
+#pragma unroll
+        for (int s = 0; s < SPT; ++s) {
+            const int i = tid + s * T;
+            if (i < V) va[i] *= inv0;
+        }
         __syncthreads();
 
         double* v1 = va;  // current Lanczos vector
@@ -173,42 +227,43 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
         bool have_drop = false;
         bool done = false, unconverged = false;
         while (!done) {
-            // w = M v1 - beta_prev v0  (into v0), alpha = <w, v1>
-            double a = 0.0;
-            for (int i = tid; i < V; i += T) {
-                const double vi = v1[i];
-                double acc = 0.0;
+            // w = M v1 - beta_prev v0 (kept in registers), alpha = <w, v1>
+            double w[SPT], vi[SPT], a = 0.0;
 #pragma unroll
-                for (int mu = 0; mu < DIM; ++mu) {
-                    const int jf = __ldg(D.fwd + i * DIM + mu), jb = __ldg(D.bwd + i * DIM + mu);
-                    acc = fma(c[mu * V + i], vi - v1[jf], acc);
-                    acc = fma(c[mu * V + jb], vi - v1[jb], acc);
+            for (int s = 0; s < SPT; ++s) {
+                const int i = tid + s * T;
+                w[s] = 0.0;
+                vi[s] = 0.0;
+                if (i < V) {
+                    vi[s] = v1[i];
+                    double acc = 0.0;
+#pragma unroll
+                    for (int mu = 0; mu < DIM; ++mu) {
+                        const int jf = nf[s][mu], jb = nb[s][mu];
+                        acc = fma(c[mu * V + i], vi[s] - v1[jf], acc);
+                        acc = fma(c[mu * V + jb], vi[s] - v1[jb], acc);
+                    }
+                    w[s] = fma(-beta_prev, v0[i], acc);
+                    a = fma(w[s], vi[s], a);
                 }
-                const double w = fma(-beta_prev, v0[i], acc);
-                v0[i] = w;
-                a = fma(w, vi, a);
             }
             a = block_sum(a, red, buf);
-            // w -= alpha v1 ; remove the constant mode ; beta = |w|
+            // w -= alpha v1; its mean (the constant mode, taken out every step) and its norm without the mean
             double sw = 0.0, sww = 0.0;
-            for (int i = tid; i < V; i += T) {
-                const double w = fma(-a, v1[i], v0[i]);
-                v0[i] = w;
-                sw += w;
+#pragma unroll
+            for (int s = 0; s < SPT; ++s) {
+                w[s] = fma(-a, vi[s], w[s]);
+                sw += w[s];
+                sww = fma(w[s], w[s], sww);
             }
-            sw = block_sum(sw, red, buf);
+            block_sum2(sw, sww, red2, buf2);
             const double mean = sw / (double)V;
-            for (int i = tid; i < V; i += T) {
-                const double w = v0[i] - mean;
-                v0[i] = w;
-                sww = fma(w, w, sww);
-            }
-            sww = block_sum(sww, red, buf);
-            const double b = sqrt(sww);
+            const double bb = fmax(fma(-(double)V * mean, mean, sww), 0.0);
+            const double b = sqrt(bb);
             if (tid == 0) {
                 alpha[k] = a;
                 beta[k] = b;
-                beta2[k] = sww;
+                beta2[k] = bb;
                 ibeta[k] = 1.0 / b;
             }
             ++k;
@@ -255,7 +310,11 @@ __global__ void __launch_bounds__(1024) lanczos_kernel(const OrbitDev D, const F
             }
             if (!done) {
                 const double ib = 1.0 / b;
-                for (int i = tid; i < V; i += T) v0[i] *= ib;
+#pragma unroll
+                for (int s = 0; s < SPT; ++s) {
+                    const int i = tid + s * T;
+                    if (i < V) v0[i] = (w[s] - mean) * ib;   // the new vector takes the place of the one before the last
+                }
                 double* tmp = v0;
                 v0 = v1;
                 v1 = tmp;
@@ -282,16 +341,19 @@ int launch(const u1gf_orbit* o, const FpParams& P, cudaStream_t st) {
     const size_t smem = ((size_t)V * DIM + 2 * (size_t)V + 4 * (size_t)(kcap > 0 ? kcap : 1)) * sizeof(double);
     if (smem > 220 * 1024)
         return fail(U1GF_EINVAL, "u1gf_check_fp: lattice of %d sites does not fit the resident Lanczos kernel", V);
-    auto kern = lanczos_kernel<DIM>;
-    if (smem > 48 * 1024) U1GF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // few threads per configuration: the Ritz test is serial work of one warp, during which the other warps of the
     // CTA wait; many small CTAs per SM keep the SM busy with other configurations meanwhile (measured: 8 warps per
     // configuration spent 54 % of their time at that barrier)
-#ifndef U1GF_FP_SITES_PER_THREAD
-#define U1GF_FP_SITES_PER_THREAD 8
-#endif
-    int T = ((V + U1GF_FP_SITES_PER_THREAD - 1) / U1GF_FP_SITES_PER_THREAD + 31) / 32 * 32;
-    if (T > 512) T = 512;
+    // sites per thread: 8 for the large lattices; fewer on the small ones, where a configuration is one or two warps and
+    // the SM needs more of them in flight to cover the latencies of the dependent chain of a Lanczos step (measured, hot
+    // orbits: 4^4 43.1 / 35.1 / 46.6 ms per 131072 copies at 8 / 4 / 2 sites per thread, 4^3 7.9 / 4.5 / 3.8 ms per 65536)
+    const int spt = V <= 128 ? 2 : (V <= 512 ? 4 : 8);
+    const int T = ((V + spt - 1) / spt + 31) / 32 * 32;
+    // the thread count bounds the registers ptxas may use
+    auto kern = spt == 8 ? (T <= 256 ? lanczos_kernel<DIM, 8, 256> : lanczos_kernel<DIM, 8, 640>)
+                         : (spt == 4 ? lanczos_kernel<DIM, 4, 256> : lanczos_kernel<DIM, 2, 256>);
+    if (T > 640) return fail(U1GF_EINVAL, "u1gf_check_fp: lattice of %d sites does not fit the resident Lanczos kernel", V);
+    if (smem > 48 * 1024) U1GF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
     U1GF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T, smem));
     if (per_sm < 1) return fail(U1GF_ECUDA, "u1gf_check_fp: kernel does not fit on an SM");
