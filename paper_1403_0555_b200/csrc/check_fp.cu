@@ -347,11 +347,14 @@ int launch(const u1gf_orbit* o, const FpParams& P, cudaStream_t st) {
     // sites per thread: 8 for the large lattices; fewer on the small ones, where a configuration is one or two warps and
     // the SM needs more of them in flight to cover the latencies of the dependent chain of a Lanczos step (measured, hot
     // orbits: 4^4 43.1 / 35.1 / 46.6 ms per 131072 copies at 8 / 4 / 2 sites per thread, 4^3 7.9 / 4.5 / 3.8 ms per 65536)
-    const int spt = V <= 128 ? 2 : (V <= 512 ? 4 : 8);
+#ifndef U1GF_FP_SPT4_MAXV
+#define U1GF_FP_SPT4_MAXV 512
+#endif
+    const int spt = V <= 128 ? 2 : (V <= U1GF_FP_SPT4_MAXV ? 4 : 8);
     const int T = ((V + spt - 1) / spt + 31) / 32 * 32;
     // the thread count bounds the registers ptxas may use
     auto kern = spt == 8 ? (T <= 256 ? lanczos_kernel<DIM, 8, 256> : lanczos_kernel<DIM, 8, 640>)
-                         : (spt == 4 ? lanczos_kernel<DIM, 4, 256> : lanczos_kernel<DIM, 2, 256>);
+                         : (spt == 4 ? (T <= 256 ? lanczos_kernel<DIM, 4, 256> : lanczos_kernel<DIM, 4, 640>) : lanczos_kernel<DIM, 2, 256>);
     if (T > 640) return fail(U1GF_EINVAL, "u1gf_check_fp: lattice of %d sites does not fit the resident Lanczos kernel", V);
     if (smem > 48 * 1024) U1GF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
