@@ -22,6 +22,12 @@
  *                            + 1 STS.128 (neighbours of 32 starts and the store), 1 = 8 warp-uniform LDS.128
  *                            (links), 2 = both (the 13 shared-memory instructions of one 4^4 site update).
  *   u1gf_measure_smem_peak   same for 128-bit conflict-free shared-memory loads, bytes per second.
+ *   u1gf_measure_dsmem_rate  thread-block clusters of `cluster_size` CTAs (512 threads, 200 KB of shared memory each --
+ *                            the footprint of a resident relaxation kernel): bytes per second and SM that a CTA pulls
+ *                            out of the shared memory of its neighbour in the cluster (remote = 1) or of its own
+ *                            through the cluster window (remote = 0) with 128-bit loads, 512 bytes per warp; and how
+ *                            many such clusters the device holds at once.  The halo exchange of a cluster-resident
+ *                            kernel for 6^4 / 8^4 would run at this rate.
  */
 #ifndef U1GF_MEASURE_H
 #define U1GF_MEASURE_H
@@ -41,6 +47,8 @@ int u1gf_measure_fp64_peak(double ms, double* dfma_per_s, void* cuda_stream);
 int u1gf_measure_fp64_rate(int32_t pattern, double ms, double* dfma_per_s, void* cuda_stream);
 int u1gf_measure_smem_peak(double ms, double* bytes_per_s, void* cuda_stream);
 int u1gf_measure_smem_rate(int32_t mix, double ms, double* instr_per_s, void* cuda_stream);
+int u1gf_measure_dsmem_rate(int32_t cluster_size, int32_t remote, double ms, double* bytes_per_s_per_sm,
+                            int32_t* max_active_clusters, void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -66,6 +66,7 @@ _MEASURE_SIGNATURES = {
     "u1gf_measure_fp64_rate": (C.c_int, [C.c_int32, C.c_double, C.POINTER(C.c_double), _p]),
     "u1gf_measure_smem_peak": (C.c_int, [C.c_double, C.POINTER(C.c_double), _p]),
     "u1gf_measure_smem_rate": (C.c_int, [C.c_int32, C.c_double, C.POINTER(C.c_double), _p]),
+    "u1gf_measure_dsmem_rate": (C.c_int, [C.c_int32, C.c_int32, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_int32), _p]),
 }
 MEASURE_LIB_PATH = os.path.join(_HERE, "libu1gf_measure.so")
 
@@ -485,6 +486,14 @@ def measure_smem_rate(mix: int, ms=200.0) -> float:
     v = C.c_double(0)
     _mcheck(measure_lib().u1gf_measure_smem_rate(int(mix), float(ms), C.byref(v), _stream()))
     return v.value
+
+
+def measure_dsmem_rate(cluster_size: int, remote: bool, ms=100.0):
+    """-> (bytes per second and SM, clusters of that size resident at once)."""
+    v, n = C.c_double(0), C.c_int32(0)
+    _mcheck(measure_lib().u1gf_measure_dsmem_rate(int(cluster_size), 1 if remote else 0, float(ms), C.byref(v), C.byref(n),
+                                                  _stream()))
+    return v.value, n.value
 
 
 def last_launch_count() -> int:

@@ -182,6 +182,38 @@ __global__ void __launch_bounds__(512) lds_mix_kernel(unsigned* out, int iters) 
     if ((acc.x ^ acc.y) == 0x12345u) out[threadIdx.x] = acc.x;
 }
 
+// Distributed shared memory (thread-block clusters): every CTA of a cluster of `csize` CTAs (512 threads, 200 KB of
+// shared memory, one CTA per SM -- the footprint of a resident relaxation kernel) pulls 512-byte rows, one 128-bit word
+// per lane, out of the shared memory of its neighbour in the cluster (REMOTE) or out of its own through the cluster
+// window.  This is the halo exchange a cluster-resident kernel for 6^4 / 8^4 would live on.
+__device__ __forceinline__ unsigned dsmem_mapa(unsigned addr, unsigned rank) {
+    unsigned r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+template <bool REMOTE>
+__global__ void __launch_bounds__(512) dsmem_kernel(double* out, int iters, int csize) {
+    extern __shared__ __align__(16) double2 dsm[];
+    unsigned rank;
+    asm("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+    for (int i = threadIdx.x; i < 12800; i += blockDim.x) dsm[i] = make_double2((double)i, (double)rank);
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;\n");
+    const unsigned base = (unsigned)__cvta_generic_to_shared(dsm);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned ra = dsmem_mapa(base + (warp * 8 * 32 + lane) * 16, REMOTE ? (rank + 1) % (unsigned)csize : rank);
+    double acc = 0.0;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int h = 0; h < 8; ++h) {
+            double2 v;
+            asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(ra + h * 512 + ((it * 37) & 15) * 4096));
+            acc += v.x + v.y;
+        }
+    }
+    if (acc == 1.2345) out[0] = acc;   // never true; keeps the loads alive
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;\n");
+}
+
 }  // namespace
 }  // namespace u1gf
 
@@ -375,6 +407,66 @@ int u1gf_measure_smem_rate(int32_t mix, double ms, double* instr_per_s, void* cu
     cudaFree(scratch);
     if (e != cudaSuccess) return fail(U1GF_ECUDA, "u1gf_measure_smem_rate: %s", cudaGetErrorString(e));
     *instr_per_s = best;
+    return U1GF_OK;
+}
+
+int u1gf_measure_dsmem_rate(int32_t cluster_size, int32_t remote, double ms, double* bytes_per_s_per_sm,
+                            int32_t* max_active_clusters, void* cuda_stream) {
+    t_launches = 0;
+    if (!bytes_per_s_per_sm || !max_active_clusters || !(ms > 0.0) || cluster_size < 1 || cluster_size > 16)
+        return fail(U1GF_EINVAL, "u1gf_measure_dsmem_rate: bad argument");
+    if (int rc = check_device()) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    auto kern = remote ? dsmem_kernel<true> : dsmem_kernel<false>;
+    const int smem = 200 * 1024;
+    U1GF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    U1GF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    cudaLaunchConfig_t cfg = {};
+    cfg.blockDim = dim3(512);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)cluster_size;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    cfg.gridDim = dim3((unsigned)cluster_size);
+    int ncl = 0;
+    U1GF_CUDA(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
+    *max_active_clusters = ncl;
+    *bytes_per_s_per_sm = 0.0;
+    if (ncl < 1) return U1GF_OK;
+    cfg.gridDim = dim3((unsigned)(cluster_size * ncl));
+    double* scratch = nullptr;
+    U1GF_CUDA(cudaMalloc(&scratch, 64));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int iters = 4000;
+    const double per_cta = (double)iters * 8.0 * 512.0 * 16.0;   // 16 warps x 8 loads x 512 bytes per iteration
+    double best = 0.0, spent = 0.0;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, scratch, 50, (int)cluster_size);   // warm-up
+    ++t_launches;
+    while (e == cudaSuccess && spent < ms) {
+        cudaEventRecord(e0, st);
+        e = cudaLaunchKernelEx(&cfg, kern, scratch, iters, (int)cluster_size);
+        cudaEventRecord(e1, st);
+        ++t_launches;
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) break;
+        float t = 0.f;
+        cudaEventElapsedTime(&t, e0, e1);
+        spent += t;
+        const double rate = per_cta / (t * 1e-3);
+        if (rate > best) best = rate;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(scratch);
+    if (e != cudaSuccess) return fail(U1GF_ECUDA, "u1gf_measure_dsmem_rate: %s", cudaGetErrorString(e));
+    *bytes_per_s_per_sm = best;
     return U1GF_OK;
 }
 

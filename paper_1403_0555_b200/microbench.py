@@ -52,6 +52,11 @@ def main() -> int:
         rate = b.measure_smem_rate(mix, 100.0)                      # warp-level instructions per second
         rows.append((label, f"{sm_cycles_per_s / rate * n:.1f} cycles / site / SM",
                      f"{sm_cycles_per_s / rate:.2f} cycles / instr / SM"))
+    for cs, remote in ((2, True), (8, True), (9, True), (16, True), (16, False)):
+        rate, ncl = b.measure_dsmem_rate(cs, remote, 60.0)
+        rows.append((f"distributed shared memory, cluster of {cs} CTAs x 512 threads x 200 KB, 128-bit loads from "
+                     f"{'the neighbour CTA' if remote else 'the own CTA through the cluster window'}",
+                     f"{rate / (mhz * 1e6):.1f} bytes / cycle / SM", f"{ncl} clusters resident ({ncl * cs} SMs)"))
     print(f"device: {props.name}, {sms} SMs, SM clock taken as {mhz:.0f} MHz\n")
     print("| probe | result | |")
     print("|---|---|---|")
