@@ -92,8 +92,8 @@ int u1gf_create_orbit(int d, const int32_t* extents, const double* theta_host, u
     auto align = [](size_t b) { return (b + 255) & ~(size_t)255; };
     const size_t bU = align((size_t)V * d * sizeof(double2)), bT = align((size_t)V * d * sizeof(int)),
                  bO = align((size_t)V * sizeof(int)), bS = align((size_t)V);
-    const size_t bL = align(lanes_links_bytes(d, D.ext));
-    o->blob_bytes = bU + 2 * bT + bO + bS + bL;
+    const size_t bL = align(lanes_links_bytes(d, D.ext)), bM = align(tma_links_bytes(d, D.ext));
+    o->blob_bytes = bU + 2 * bT + bO + bS + bL + bM;
     cudaGetDevice(&o->device);
     cudaDeviceGetAttribute(&o->sm_count, cudaDevAttrMultiProcessorCount, o->device);
     cudaError_t e = cudaMalloc(&o->blob, o->blob_bytes);
@@ -126,6 +126,11 @@ int u1gf_create_orbit(int d, const int32_t* extents, const double* theta_host, u
         o->U_lanes = (const double2*)(dptr + off);
         o->U_lanes_host.assign((const double2*)(h + off), (const double2*)(h + off) + (size_t)V * d);
     }
+    off += bL;
+    if (bM) {
+        tma_fill_links(o, (double2*)(h + off));
+        o->U_tma = (const double2*)(dptr + off);
+    }
     e = cudaMemcpy(o->blob, h, o->blob_bytes, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
         cudaFree(o->blob);
@@ -145,20 +150,24 @@ int u1gf_destroy_orbit(u1gf_orbit* o) {
 }
 
 int u1gf_set_kernel(u1gf_orbit* o, int32_t which) {
-    if (!o || which < 0 || which > 2) return fail(U1GF_EINVAL, "u1gf_set_kernel: bad argument");
+    if (!o || which < 0 || which > 3) return fail(U1GF_EINVAL, "u1gf_set_kernel: bad argument");
     o->kernel_choice = which;
     return U1GF_OK;
 }
 
 static bool use_lanes(const u1gf_orbit* o) { return o->kernel_choice == 0 && lanes_supported(o); }
+static bool use_tma(const u1gf_orbit* o) {
+    return !use_lanes(o) && (o->kernel_choice == 0 || o->kernel_choice == 3) && tma_supported(o);
+}
 static bool use_stream(const u1gf_orbit* o) {
-    if (use_lanes(o)) return false;
+    if (use_lanes(o) || use_tma(o)) return false;
     return (o->kernel_choice == 0 && stream_preferred(o)) || (o->kernel_choice == 2 && stream_supported(o));
 }
 
 const char* u1gf_kernel_name(const u1gf_orbit* o) {
     if (!o) return "";
     return use_lanes(o)    ? lanes_name(o)
+           : use_tma(o)    ? "tma_stream_lane_per_start"
            : use_stream(o) ? (o->dev.all_even ? "stream_lane_per_start" : "phased_lane_per_start")
                            : "generic_cta_per_start";
 }
@@ -166,6 +175,7 @@ const char* u1gf_kernel_name(const u1gf_orbit* o) {
 size_t u1gf_relax_workspace_bytes(const u1gf_orbit* o, uint64_t n_starts) {
     if (!o) return 0;
     return use_lanes(o)    ? lanes_workspace_bytes(o, n_starts)
+           : use_tma(o)    ? tma_workspace_bytes(o, n_starts)
            : use_stream(o) ? stream_workspace_bytes(o, n_starts)
                            : generic_workspace_bytes(o, n_starts);
 }
@@ -191,7 +201,10 @@ int u1gf_relax_batch(const u1gf_orbit* o, uint64_t seed, uint64_t first_start, u
     RelaxArgs a{seed, first_start, n_starts, start_ids, omega, eps, max_sweeps, check_every,
                 F_norm, sweeps, status, sig, g_canon, workspace, workspace_bytes};
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    return use_lanes(o) ? lanes_relax(o, a, st) : use_stream(o) ? stream_relax(o, a, st) : generic_relax(o, a, st);
+    return use_lanes(o)    ? lanes_relax(o, a, st)
+           : use_tma(o)    ? tma_relax(o, a, st)
+           : use_stream(o) ? stream_relax(o, a, st)
+                           : generic_relax(o, a, st);
 }
 
 }  // extern "C"

@@ -103,10 +103,12 @@ struct u1gf_orbit {
     size_t blob_bytes = 0;
     int device = 0;
     int sm_count = 0;
-    int kernel_choice = 0;  // 0 auto, 1 generic, 2 streamed (falls back to generic where it does not apply)
+    int kernel_choice = 0;  // 0 auto, 1 generic, 2 streamed with plain loads, 3 TMA-staged streamed (2, 3 fall back to generic where they do not apply)
     // device copy of the links in the layout of the specialised resident kernels (inside blob), or null
     const double2* U_lanes = nullptr;
     std::vector<double2> U_lanes_host;  // host copy of the links part of that table (kernel parameter of the NB == 1 kernels)
+    // device copy of the links in the row order of the TMA-staged streamed kernel (inside blob), or null
+    const double2* U_tma = nullptr;
 };
 
 namespace u1gf {
@@ -151,5 +153,12 @@ bool stream_supported(const u1gf_orbit* o);   // every extent even
 bool stream_preferred(const u1gf_orbit* o);   // ... and large enough to be the automatic choice
 size_t stream_workspace_bytes(const u1gf_orbit* o, uint64_t n);
 int stream_relax(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st);
+
+// TMA-staged streamed kernel for 6^4 and 8^4 (relax_tma.cu)
+size_t tma_links_bytes(int d, const int* ext);   // extra blob bytes for its link table (0 if the extents have no such kernel)
+void tma_fill_links(const u1gf_orbit* o, double2* dst_host);
+bool tma_supported(const u1gf_orbit* o);
+size_t tma_workspace_bytes(const u1gf_orbit* o, uint64_t n);
+int tma_relax(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st);
 
 }  // namespace u1gf

@@ -67,8 +67,8 @@ def test_relax_matches_oracle(b, oracle, ext, seed, n, kernel):
     odd = any(e % 2 for e in ext)
     if kernel == 2 and orbit.kernel_name != ("phased_lane_per_start" if odd else "stream_lane_per_start"):
         pytest.fail("set_kernel(2) must select the streamed (all-even) / phased (odd extent) lane-per-start kernel")
-    if kernel == 0 and orbit.V >= 1024 and not odd:
-        assert orbit.kernel_name == "stream_lane_per_start"
+    if kernel == 0 and orbit.V >= 1024 and not odd:   # 6^4, 8^4: the TMA-staged streamed kernel
+        assert orbit.kernel_name == ("tma_stream_lane_per_start" if ext in ((6,) * 4, (8,) * 4) else "stream_lane_per_start")
     if kernel == 0 and orbit.V >= 64 and odd:
         assert orbit.kernel_name == "phased_lane_per_start"
     V = orbit.V
