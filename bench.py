@@ -170,10 +170,12 @@ class Pipeline:
         name = self.orbit.kernel_name
         roof = {"bound": "alu", "achieved": fp64, "peak": peak, "unit": "TFLOP/s", "frac": fp64 / peak,
                 "frac_of_fp64_pipe": fp64 / pipe, "fp64_pipe_peak": pipe, "traffic": None}
-        if name.startswith("stream"):
+        if name.startswith("stream") or name.startswith("tma_stream"):
+            # 32 B of HBM per site update (g read + written once per sweep).  The checkerboard as built moves
+            # 48 B (the rows of a parity are read twice per sweep: as neighbours and as the site itself), DESIGN.md 7.4
             gbs = su * 32.0 / (relax_ms * 1e-3) / 1e9
             roof = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
-                    "fp64_frac": fp64 / peak, "traffic": None}
+                    "frac_at_48_bytes_moved": gbs * 1.5 / hbm_peak, "fp64_frac": fp64 / peak, "traffic": None}
         roof.update(kernel=name, kernel_ms=relax_ms, kernel_share_of_step=relax_ms / step_ms)
         return dict(workload=f"{'x'.join(map(str, self.ext))} seed {self.seed}, {self.n} starts", value=su / (step_ms * 1e-3),
                     ms_per_step=step_ms, relax_kernel_ms=relax_ms, first_region_ms=fp_ms,

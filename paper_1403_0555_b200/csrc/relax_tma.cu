@@ -9,8 +9,8 @@
 // that a producer warp issues several tiles ahead, completion counted by mbarriers, and the consumer warps read them
 // with conflict-free LDS.128.  The data in flight sits in shared memory (about 100 KB per SM), not in registers.
 //
-// Layout of a team's field (workspace): three arrays O (odd sites), E0, E1 (even sites, double buffered for the stop
-// rule R5), each [sheet = x3*N + x2][x1][k][32 starts] double2, where the half-line (x1, x2, x3) of parity p holds
+// Layout of a team's field (workspace): three arrays O (odd sites), E (even sites) and SV (the pre-update even values
+// of the lanes that may stop at this sweep, see below), each [sheet = x3*N + x2][x1][k][32 starts] double2, where the half-line (x1, x2, x3) of parity p holds
 // the sites x0 = 2k + ((p + x1 + x2 + x3) & 1), k = 0 .. N/2-1.  A "half-sheet" (all x0, x1 of one parity at fixed
 // x2, x3) is one contiguous block of N * N/2 rows = 16 KB at N = 8, 9 KB at N = 6: the unit of a bulk copy.
 //
@@ -41,7 +41,7 @@ struct TmaParams {
     uint8_t* status;
     double* sig;
     double* g_canon;
-    double2* team_buf;             // [teams][3][V/2][32]: O, E0, E1
+    double2* team_buf;             // [teams][3][V/2][32]: O, E, SV
     const double2* lnk;            // [2][V/2][8]: links in row order, forward U_{i,mu} then backward U_{i-mu,mu}
     unsigned long long* counter;   // next start position to hand out
     OrbitDev D;
@@ -51,22 +51,38 @@ template <int N>
 struct TG {
     static constexpr int H = N / 2;            // rows of a half-line
     static constexpr int SITES = N * H;        // sites of one parity in a sheet = sites per step
-    static constexpr int SPW = SITES % 16 == 0 ? SITES / 16 : 1;   // sites per consumer warp and step
-    static constexpr int CW = SITES / SPW;     // consumer warps (8^4: 16 x 2 sites, 6^4: 18 x 1 site)
+#ifndef U1GF_TMA_SPW8
+#define U1GF_TMA_SPW8 4
+#endif
+#ifndef U1GF_TMA_SPW6
+#define U1GF_TMA_SPW6 3
+#endif
+    static constexpr int SPW = N == 8 ? U1GF_TMA_SPW8 : U1GF_TMA_SPW6;   // sites per consumer warp and step (knobs: 8^4: 4, 2, 1; 6^4: 3, 1)
+    static constexpr int CW = SITES / SPW;     // consumer warps (8^4: 8 x a half-line of 4 sites, 6^4: 6 x a half-line of 3)
     static constexpr int THREADS = (CW + 1) * 32;   // + the producer warp
     static constexpr int V = N * N * N * N, HALF = V / 2;
     static constexpr int NS = N * N;           // steps per half-sweep
     static constexpr int WL = N * (N + 2);     // window fetches per half-sweep
-    static constexpr int RW = 6;               // window slots
-    static constexpr int ST = N >= 8 ? 3 : 4;  // stages of the x3-neighbour / link ring
-    static constexpr int LA = 2;               // steps the window fetches run ahead
+#ifndef U1GF_TMA_ST6
+#define U1GF_TMA_ST6 4
+#endif
+#ifndef U1GF_TMA_RW6
+#define U1GF_TMA_RW6 6
+#endif
+#ifndef U1GF_TMA_LA6
+#define U1GF_TMA_LA6 2
+#endif
+    static constexpr int RW = N >= 8 ? 6 : U1GF_TMA_RW6;          // window slots
+    static constexpr int ST = N >= 8 ? 3 : U1GF_TMA_ST6;          // stages of the x3-neighbour / link ring
+    static constexpr int LA = N >= 8 ? 2 : U1GF_TMA_LA6;          // steps the window fetches run ahead
+    static constexpr unsigned HSMOD = 4 * RW * ST;
     static constexpr unsigned SHEET_B = SITES * 512, LNK_B = SITES * 128;
     static constexpr size_t off_win = 0;
     static constexpr size_t off_x3 = off_win + (size_t)RW * SHEET_B;
     static constexpr size_t off_lnk = off_x3 + (size_t)ST * 2 * SHEET_B;
     static constexpr size_t off_bar = off_lnk + (size_t)ST * LNK_B;           // fullW[RW], fullS[ST], empty[ST]
     static constexpr size_t off_sred = off_bar + (size_t)(RW + 2 * ST) * 8 + 8;
-    static constexpr size_t off_red = off_sred + (size_t)2 * CW * 32 * 8;
+    static constexpr size_t off_red = off_sred + (size_t)3 * CW * 32 * 8;   // [2][CW][32] sweep sums, [CW][32] odd sums
     static constexpr size_t off_pos = off_red + (size_t)2 * (CW + 1) * 5 * 8;
     static constexpr size_t off_skip = off_pos + 32 * 8;
     static constexpr size_t smem_bytes = off_skip + 32 * 4 + 16;
@@ -130,14 +146,13 @@ __device__ __forceinline__ void block_sum(double (&v)[NV], double* red, int& buf
     buf ^= 1;
 }
 
-__device__ __noinline__ bool r6_vanishes(double nw) {
-    return (unsigned long long)__double_as_longlong(nw) < (unsigned long long)__double_as_longlong(1e-280);
-}
-
 // a3 for one site of one start: g <- normalise((1-omega) g + omega w/|w|) (R2), the 8d+20 form of
 // relax_lanes.cu (h' = g + (k2/|w|) w = h/(1-omega), second-order rsqrt polish); W1: omega == 1, g <- w/|w|.
+// R6 (|w|^2 < 1e-280: the site keeps its value) by selects, not a branch: the sites a warp updates in one step then
+// form ONE basic block and ptxas interleaves their dependent chains (with the branch, each site ran alone and the warp
+// issued one instruction every 5 cycles).
 template <bool W1>
-__device__ __forceinline__ double2 site_update(double2 g, double wr, double wi, double k2, bool& skipped) {
+__device__ __forceinline__ double2 site_update(double2 g, double wr, double wi, double k2, bool& small) {
     const double nw = fma(wr, wr, wi * wi);
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(nw));
@@ -156,12 +171,10 @@ __device__ __forceinline__ double2 site_update(double2 g, double wr, double wi, 
         const double r2 = fma(y2 * -0.5, e2, -y2);
         gn = make_double2(hr * r2, hi * r2);
     }
-    if (__double2hiint(nw) <= __double2hiint(1e-280)) {   // R6
-        if (r6_vanishes(nw)) {
-            gn = g;
-            skipped = true;
-        }
-    }
+    // bit patterns of non-negative doubles are ordered like the numbers
+    small = (unsigned long long)__double_as_longlong(nw) < (unsigned long long)__double_as_longlong(1e-280);
+    gn.x = small ? g.x : gn.x;
+    gn.y = small ? g.y : gn.y;
     return gn;
 }
 
@@ -174,27 +187,35 @@ __device__ __forceinline__ void locate(int i, int& p, int& row) {
     row = l * (N / 2) + (x0 >> 1);
 }
 
+#ifdef U1GF_TMA_PROF   // debugging knob: cycle counters of CTA 0 printed at the end of the kernel
+__device__ unsigned long long g_prof[16];
+#define PROF_T0() const long long prof_t0 = clock64()
+#define PROF_ADD(k) if (blockIdx.x == 0 && lane == 0) atomicAdd(&g_prof[k], (unsigned long long)(clock64() - prof_t0))
+#else
+#define PROF_T0()
+#define PROF_ADD(k)
+#endif
+
 template <int N>
 struct Smem {
     unsigned win, x3, lnk, fullW, fullS, empty;   // shared-space addresses
+    const unsigned char* base;                    // the dynamic shared memory as a generic pointer
 };
 
-// One half-sweep of parity PAR.  src / dst: rows of parity PAR before / after the update (the same array for the odd
-// half-sweep); oth: rows of the other parity; lnk: links of the parity-PAR sites in row order.  `hs` counts the
+// One half-sweep of parity PAR.  src / dst: rows of parity PAR before / after the update (the same array); save: where
+// the lanes with `cand` set keep their pre-update values (even half-sweep); oth: rows of the other parity; lnk: links of the parity-PAR sites in row order.  `hs` counts the
 // half-sweeps of this CTA (the mbarrier phases follow from it).  Returns sum Delta_i^2 over this warp's sites for the
 // lane's start: PAR == 0 measured before the update (field after the previous sweep), PAR == 1 after it.
 template <int N, int PAR, bool W1>
-__device__ __forceinline__ double half_sweep(const Smem<N>& S, const double2* __restrict__ src, double2* __restrict__ dst,
+__device__ __forceinline__ double half_sweep(const Smem<N>& S, const double2* src, double2* dst, double2* save,
                                              const double2* __restrict__ oth, const double2* __restrict__ lnk, unsigned hs,
-                                             int warp, int lane, double k2, bool commit, bool& skipped) {
+                                             int warp, int lane, double k2, bool commit, bool cand, bool& skipped) {
     using G = TG<N>;
     constexpr int H = G::H, SITES = G::SITES, SPW = G::SPW, CW = G::CW, NS = G::NS, WL = G::WL, RW = G::RW, ST = G::ST;
     const unsigned step0 = hs * NS, wl0 = hs * WL;
     double acc = 0.0;
-    // rows written by this CTA with ordinary stores (last half-sweep, refill) must be visible to the bulk copies
-    fence_proxy_async();
-    __syncthreads();
-
+    // (the caller has put fence.proxy.async + a CTA barrier in front: rows written by this CTA with ordinary stores --
+    // last half-sweep, refill -- must be visible to the bulk copies)
     if (warp == CW) {
         // ------------------------------------------------------------------ producer: one lane issues every bulk copy
         if (lane == 0) {
@@ -202,16 +223,22 @@ __device__ __forceinline__ double half_sweep(const Smem<N>& S, const double2* __
             for (int g = 0; g < NS; ++g) {
                 if (g > 0) {   // steps up to g-1 are finished by every consumer warp
                     const unsigned sg = step0 + g - 1;
+                    PROF_T0();
                     mbar_wait(S.empty + (sg % ST) * 8, (sg / ST) & 1u);
+                    PROF_ADD(0);
                 }
                 // x3 neighbours and links of the steps below g + ST: the stage of step s was last used by step s - ST
                 while (nsl < NS && nsl < g + ST) {
                     const int x3 = nsl / N, x2 = nsl % N;
                     const unsigned sg = step0 + nsl, st = sg % ST, bar = S.fullS + st * 8;
+#ifdef U1GF_TMA_ABL_NOX3   // ablation knob (wrong results): the x3 neighbours are not fetched (52 instead of 84 B per site update)
+                    mbar_expect_tx(bar, G::LNK_B);
+#else
                     mbar_expect_tx(bar, 2 * G::SHEET_B + G::LNK_B);
                     const int dn = ((x3 + N - 1) % N) * N + x2, up = ((x3 + 1) % N) * N + x2;
                     bulk_g2s(S.x3 + (st * 2 + 0) * G::SHEET_B, oth + (size_t)dn * SITES * 32, G::SHEET_B, bar);
                     bulk_g2s(S.x3 + (st * 2 + 1) * G::SHEET_B, oth + (size_t)up * SITES * 32, G::SHEET_B, bar);
+#endif
                     bulk_g2s(S.lnk + st * G::LNK_B, lnk + (size_t)nsl * SITES * 8, G::LNK_B, bar);
                     ++nsl;
                 }
@@ -237,50 +264,90 @@ __device__ __forceinline__ double half_sweep(const Smem<N>& S, const double2* __
     }
 
     // ---------------------------------------------------------------------- consumers: SPW sites per warp and step
-    const int q0 = warp * SPW;   // first site of this warp inside a half-sheet, q = x1 * H + k
-    double2 own[SPW], nxt[SPW];
+    // Per-step bookkeeping is kept incremental and everything that depends only on the warp's sites is formed once:
+    // with SPW sites per warp and step every instruction outside the site update is paid SPW times less often.
+    // ordinary shared-memory loads (offsets from the start of the dynamic shared memory): the mbarrier waits are asm
+    // statements with a memory clobber, so the compiler keeps these loads behind them and is otherwise free to schedule
+    auto lds = [&](unsigned off) { return *reinterpret_cast<const double2*>(S.base + off); };
+    constexpr bool LINE = SPW == H;   // a warp owns a whole half-line: its H rows of the other parity serve all x0 neighbours
+    const int q0 = warp * SPW;        // first site of this warp inside a half-sheet, q = x1 * H + k
+    const unsigned l16 = lane * 16;
+    unsigned vF0[SPW][2], vB0[SPW][2], vF1[SPW], vB1[SPW], vQ[SPW];   // byte offsets inside a half-sheet (+ the lane's 16 bytes)
+    unsigned vRow[LINE ? H : 1];
+    int abase[SPW];
 #pragma unroll
-    for (int j = 0; j < SPW; ++j) own[j] = __ldcs(src + (size_t)(q0 + j) * 32 + lane);
-    for (int g = 0; g < NS; ++g) {
-        const int x3 = g / N, x2 = g % N;
+    for (int j = 0; j < SPW; ++j) {
+        const int q = q0 + j, x1 = q / H, k = q % H;
+        const int x1f = x1 + 1 == N ? 0 : x1 + 1, x1b = x1 == 0 ? N - 1 : x1 - 1;
+#pragma unroll
+        for (int a = 0; a < 2; ++a) {   // x0 = 2k + a
+            const int kf = a ? (k + 1 == H ? 0 : k + 1) : k, kb = a ? k : (k == 0 ? H - 1 : k - 1);
+            vF0[j][a] = (x1 * H + kf) * 512 + l16;
+            vB0[j][a] = (x1 * H + kb) * 512 + l16;
+        }
+        vF1[j] = (x1f * H + k) * 512 + l16;
+        vB1[j] = (x1b * H + k) * 512 + l16;
+        vQ[j] = q * 512 + l16;
+        abase[j] = (PAR + x1) & 1;
+        if (LINE) vRow[LINE ? j : 0] = vQ[j];
+    }
+    double2 own[SPW], nxt[SPW];
+    const double2* psrc = src + (size_t)q0 * 32 + lane;
+    double2* pdst = dst + (size_t)q0 * 32 + lane;
+#pragma unroll
+    for (int j = 0; j < SPW; ++j) own[j] = __ldcs(psrc + j * 32);
+    // ring positions of step 0: window fetch of the x2-1 half-sheet (slot, phase parity), stage (index, phase parity)
+    unsigned sDn = wl0 % RW, pDn = (wl0 / RW) & 1u, st = step0 % ST, pst = (step0 / ST) & 1u;
+    int x2 = 0, sp = 0;   // sp = (x2 + x3) & 1
+    auto step = [&](int g, double2 (&own)[SPW], double2 (&nxt)[SPW]) {
+        psrc += SITES * 32;
         if (g + 1 < NS) {
 #pragma unroll
-            for (int j = 0; j < SPW; ++j) nxt[j] = __ldcs(src + ((size_t)(g + 1) * SITES + q0 + j) * 32 + lane);
+            for (int j = 0; j < SPW; ++j) nxt[j] = __ldcs(psrc + j * 32);
         }
-        const unsigned gw = wl0 + x3 * (N + 2) + x2, sg = step0 + g, st = sg % ST;
-        const unsigned sDn = gw % RW, sC = (gw + 1) % RW, sUp = (gw + 2) % RW;
-        mbar_wait(S.fullW + sDn * 8, (gw / RW) & 1u);
-        mbar_wait(S.fullW + sC * 8, ((gw + 1) / RW) & 1u);
-        mbar_wait(S.fullW + sUp * 8, ((gw + 2) / RW) & 1u);
-        mbar_wait(S.fullS + st * 8, (sg / ST) & 1u);
-        const unsigned bC = S.win + sC * G::SHEET_B + lane * 16, bDn2 = S.win + sDn * G::SHEET_B + lane * 16,
-                       bUp2 = S.win + sUp * G::SHEET_B + lane * 16;
-        const unsigned bDn3 = S.x3 + (st * 2) * G::SHEET_B + lane * 16, bUp3 = bDn3 + G::SHEET_B;
-        const unsigned bL = S.lnk + st * G::LNK_B;
-        auto lds = [](unsigned a) {
-            double2 v;
-            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
-            return v;
-        };
+        unsigned sC = sDn + 1, pC = pDn;
+        if (sC == RW) sC = 0, pC ^= 1u;
+        unsigned sUp = sC + 1, pUp = pC;
+        if (sUp == RW) sUp = 0, pUp ^= 1u;
+        PROF_T0();
+        if (x2 == 0) {   // first step of a layer: all three half-sheets are new; later ones were waited for as C / Up
+            mbar_wait(S.fullW + sDn * 8, pDn);
+            mbar_wait(S.fullW + sC * 8, pC);
+        }
+        mbar_wait(S.fullW + sUp * 8, pUp);
+        mbar_wait(S.fullS + st * 8, pst);
+        if (warp == 0) { PROF_ADD(1); }
+        const unsigned bC = (unsigned)G::off_win + sC * G::SHEET_B, bDn2 = (unsigned)G::off_win + sDn * G::SHEET_B,
+                       bUp2 = (unsigned)G::off_win + sUp * G::SHEET_B;
+        const unsigned bDn3 = (unsigned)G::off_x3 + (st * 2) * G::SHEET_B, bUp3 = bDn3 + G::SHEET_B;
+        const unsigned bL = (unsigned)G::off_lnk + st * G::LNK_B + q0 * 128;
+        double2 cf[LINE ? H : 1];
+        if (LINE) {   // cf[k] = row (k + a) mod H of the warp's line: x0+1 neighbour of site k, x0-1 neighbour of site k+1
+            const int a = abase[0] ^ sp;
+#pragma unroll
+            for (int k = 0; k < H; ++k) cf[LINE ? k : 0] = lds(bC + (a ? vRow[LINE ? (k + 1) % H : 0] : vRow[LINE ? k : 0]));
+        }
 #pragma unroll
         for (int j = 0; j < SPW; ++j) {
-            const int q = q0 + j, x1 = q / H, k = q % H;
-            const int a = (PAR + x1 + x2 + x3) & 1;   // x0 = 2k + a
-            const int kf = a ? (k + 1 == H ? 0 : k + 1) : k, kb = a ? k : (k == 0 ? H - 1 : k - 1);
-            const int x1f = x1 + 1 == N ? 0 : x1 + 1, x1b = x1 == 0 ? N - 1 : x1 - 1;
+            const int a = abase[j] ^ sp;
             double2 gf[4], gb[4], uf[4], ub[4];
-            gf[0] = lds(bC + (x1 * H + kf) * 512);
-            gb[0] = lds(bC + (x1 * H + kb) * 512);
-            gf[1] = lds(bC + (x1f * H + k) * 512);
-            gb[1] = lds(bC + (x1b * H + k) * 512);
-            gf[2] = lds(bUp2 + q * 512);
-            gb[2] = lds(bDn2 + q * 512);
-            gf[3] = lds(bUp3 + q * 512);
-            gb[3] = lds(bDn3 + q * 512);
+            if (LINE) {
+                gf[0] = cf[LINE ? j : 0];
+                gb[0] = cf[LINE ? (j + H - 1) % H : 0];
+            } else {
+                gf[0] = lds(bC + (a ? vF0[j][1] : vF0[j][0]));
+                gb[0] = lds(bC + (a ? vB0[j][1] : vB0[j][0]));
+            }
+            gf[1] = lds(bC + vF1[j]);
+            gb[1] = lds(bC + vB1[j]);
+            gf[2] = lds(bUp2 + vQ[j]);
+            gb[2] = lds(bDn2 + vQ[j]);
+            gf[3] = lds(bUp3 + vQ[j]);
+            gb[3] = lds(bDn3 + vQ[j]);
 #pragma unroll
             for (int mu = 0; mu < 4; ++mu) {
-                uf[mu] = lds(bL + (q * 8 + mu) * 16);
-                ub[mu] = lds(bL + (q * 8 + 4 + mu) * 16);
+                uf[mu] = lds(bL + (j * 8 + mu) * 16);
+                ub[mu] = lds(bL + (j * 8 + 4 + mu) * 16);
             }
             double wr = 0.0, wi = 0.0;
 #pragma unroll
@@ -299,22 +366,37 @@ __device__ __forceinline__ double half_sweep(const Smem<N>& S, const double2* __
                 const double dl = fma(gi.y, wr, -gi.x * wi);   // Delta_i of the field after sweep t
                 acc = fma(dl, dl, acc);
             }
-            bool sk = false;
+            bool sk;
             const double2 gn = site_update<W1>(gi, wr, wi, k2, sk);
-            if (commit) {
-                __stcs(dst + ((size_t)g * SITES + q) * 32 + lane, gn);
-                if (PAR == 1) {
-                    const double dl = fma(gn.y, wr, -gn.x * wi);   // Delta_i = Im(g_i conj w_i) after the update
-                    acc = fma(dl, dl, acc);
-                }
-                skipped |= sk;
+            if (PAR == 0 && cand) save[(pdst - dst) + j * 32] = gi;   // R5: a lane that may stop keeps its pre-update value
+            if (commit) __stcs(pdst + j * 32, gn);
+            if (PAR == 1) {   // (a lane without commit drops the sum below)
+                const double dl = fma(gn.y, wr, -gn.x * wi);   // Delta_i = Im(g_i conj w_i) after the update
+                acc = fma(dl, dl, acc);
             }
+            skipped |= sk && commit;
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(S.empty + st * 8);   // this warp no longer reads the buffers of step g
-#pragma unroll
-        for (int j = 0; j < SPW; ++j) own[j] = nxt[j];
+        pdst += SITES * 32;
+        // next step: the window advances by one fetch inside a layer and by three at a layer boundary (N + 2 fetches per layer)
+        if (++st == ST) st = 0, pst ^= 1u;
+        if (++x2 == N) {
+            x2 = 0;   // x2: N-1 -> 0 and x3 + 1: the sheet parity stays
+            sDn += 3;
+        } else {
+            sp ^= 1;
+            sDn += 1;
+        }
+        if (sDn >= RW) sDn -= RW, pDn ^= 1u;
+    };
+    // two steps per iteration: the rows fetched for the next step land in the other register set (no copies, so the
+    // load has a whole step to arrive)
+    for (int g = 0; g < NS; g += 2) {
+        step(g, own, nxt);
+        step(g + 1, nxt, own);
     }
+    if (PAR == 1 && !commit) acc = 0.0;
     return acc;
 }
 
@@ -325,6 +407,7 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
     constexpr int V = G::V, HALF = G::HALF, CW = G::CW, NW = CW + 1, THREADS = G::THREADS;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* sred = reinterpret_cast<double*>(smem_raw + G::off_sred);              // [2][CW][32]
+    double* sredO = sred + 2 * CW * 32;                                            // [CW][32]
     double* red = reinterpret_cast<double*>(smem_raw + G::off_red);                // [2][NW][5]
     unsigned long long* s_pos = reinterpret_cast<unsigned long long*>(smem_raw + G::off_pos);
     unsigned* s_skip = reinterpret_cast<unsigned*>(smem_raw + G::off_skip);
@@ -332,11 +415,17 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
     const OrbitDev& D = P.D;
     const int tid = threadIdx.x, lane = tid & 31, warp = __shfl_sync(FULL, tid >> 5, 0);
     double2* const O = P.team_buf + (size_t)blockIdx.x * 3 * HALF * 32;
-    double2* const E0 = O + (size_t)HALF * 32;
-    double2* const E1 = E0 + (size_t)HALF * 32;
-    auto evn = [&](int buf) { return buf ? E1 : E0; };
+    double2* const E = O + (size_t)HALF * 32;
+    // Stop rule R5: the decision on sweep t needs the even-site Delta formed by the even half-sweep of sweep t+1, and a
+    // start that stops must keep the even values from BEFORE that half-sweep.  The LDG kernel double-buffers the even
+    // rows for this; here only the lanes that can stop at this sweep -- the odd part of the gauge precision is already
+    // below eps (a necessary condition), or max_sweeps is reached -- save their old even values to SV (16-byte stores of
+    // one or two lanes per row), and the even rows are updated in place.  A team then cycles through 2 x V/2 rows
+    // instead of 3: 648 KB at 6^4, 96 MB over 148 teams, which stays in the 126 MB L2.
+    double2* const SV = E + (size_t)HALF * 32;
 
     Smem<N> S;
+    S.base = smem_raw;
     S.win = smem_u32(smem_raw + G::off_win);
     S.x3 = smem_u32(smem_raw + G::off_x3);
     S.lnk = smem_u32(smem_raw + G::off_lnk);
@@ -354,31 +443,33 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
     __syncthreads();
 
     bool active = false, fresh = false, maxed = false, skipped = false;
-    int t = 0, eb = 0, rb = 0, fb = 0;
+    int t = 0, rb = 0, fb = 0;
     unsigned hs = 0;
     double accO = 0.0;
     unsigned need = FULL, dumpm = 0;   // first pass: every lane needs a start, nothing to finalise
 
     for (;;) {
         // ---------------------------------------------------------- service (CTA-uniform): finalise, refill
+#ifdef U1GF_TMA_PROF
+        const long long prof_s0 = clock64();
+#endif
         for (unsigned m = need; m; m &= m - 1) {
             const int L = __ffs(m) - 1;
             if ((dumpm >> L) & 1u) {
-                // a5, a6 for the start of lane L: even rows before the last even half-sweep (E[eb]), odd rows O
+                // a5, a6 for the start of lane L: even rows before the last even half-sweep (saved in SV), odd rows O
                 if (skipped) atomicOr(&s_skip[lane], 1u);
                 const int tL = __shfl_sync(FULL, t, L);
                 const int mxL = __shfl_sync(FULL, maxed ? 1 : 0, L);
                 const unsigned long long k = s_pos[L];
-                const double2* E = evn(eb);
                 int pc, rc;
                 locate<N>(V - 1, pc, rc);
-                const double2 c = (pc ? O : E)[(size_t)rc * 32 + L];
+                const double2 c = (pc ? O : SV)[(size_t)rc * 32 + L];
                 double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
                 for (int i = tid; i < V; i += THREADS) {
                     int pi, ri;
                     locate<N>(i, pi, ri);
-                    const double2 gi = (pi ? O : E)[(size_t)ri * 32 + L];
-                    const double2* Nb = pi ? E : O;   // neighbours have the other parity
+                    const double2 gi = (pi ? O : SV)[(size_t)ri * 32 + L];
+                    const double2* Nb = pi ? SV : O;   // neighbours have the other parity
 #pragma unroll
                     for (int mu = 0; mu < 4; ++mu) {   // F = sum Re(g_i U_{i,mu} conj g_{i+mu})   (Eq. 3)
                         const double2 u = __ldg(D.U + i * 4 + mu);
@@ -412,7 +503,6 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
             const unsigned long long k = s_k;
             if (k < P.n_starts) {
                 const uint64_t s = P.start_ids ? P.start_ids[k] : P.first_start + k;
-                double2* En = evn(eb ^ 1);   // where the next even half-sweep looks for its own sites
                 for (int i = tid; i < V; i += THREADS) {   // a2: Philox counter (site, start lo, start hi, 0)
                     const u32x4 r = philox((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 0u, (uint32_t)P.seed,
                                            (uint32_t)(P.seed >> 32));
@@ -420,7 +510,7 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
                     sincospi(unit_interval_pm1(r.x, r.y), &sn, &cs);
                     int pi, ri;
                     locate<N>(i, pi, ri);
-                    (pi ? O : En)[(size_t)ri * 32 + L] = make_double2(cs, sn);
+                    (pi ? O : E)[(size_t)ri * 32 + L] = make_double2(cs, sn);
                 }
                 if (tid == 0) {
                     s_pos[L] = k;
@@ -437,24 +527,38 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
             }
             __syncthreads();
         }
+#ifdef U1GF_TMA_PROF
+        if (blockIdx.x == 0 && tid == 0) atomicAdd(&g_prof[3], (unsigned long long)(clock64() - prof_s0));
+#endif
         if (__ballot_sync(FULL, active) == 0) break;   // every warp holds the same lane states
 
         // ---------------------------------------------------------- odd half-sweep (second half of sweep t+1)
         {
             const bool commit = active && !fresh;
-            accO = half_sweep<N, 1, W1>(S, O, O, evn(eb ^ 1), P.lnk + (size_t)HALF * 8, hs, warp, lane, P.k2, commit, skipped);
-            hs = (hs + 1) % 12;   // the mbarrier phases only need hs modulo 12 (12 x WL, 12 x NS are multiples of 2 RW, 2 ST)
+            fence_proxy_async();
+            __syncthreads();
+            PROF_T0();
+            accO = half_sweep<N, 1, W1>(S, O, O, nullptr, E, P.lnk + (size_t)HALF * 8, hs, warp, lane, P.k2, commit, false, skipped);
+            if (warp == 0) { PROF_ADD(2); }
+            hs = (hs + 1) % G::HSMOD;   // the mbarrier phases only need hs modulo a multiple of 2 RW and 2 ST
             if (commit) ++t;
             fresh = false;
-            eb ^= 1;
         }
         // ---------------------------------------------------------- even half-sweep (first half of sweep t+1)
-        const double accE = half_sweep<N, 0, W1>(S, evn(eb), evn(eb ^ 1), O, P.lnk, hs, warp, lane, P.k2, active, skipped);
-        hs = (hs + 1) % 12;
-        // a4: gauge precision of the field after sweep t (R5), fixed summation order over the warps
-        if (warp < CW) sred[(rb * CW + warp) * 32 + lane] = accE + accO;
+        // lanes that can stop at this sweep (necessary conditions, known before the half-sweep): they save their even values
+        if (warp < CW) sredO[warp * 32 + lane] = accO;
+        fence_proxy_async();
         __syncthreads();
-        double Ssum = 0.0;
+        double sumO = 0.0;   // odd part of the gauge precision of the field after sweep t, fixed order
+#pragma unroll
+        for (int w = 0; w < CW; ++w) sumO += sredO[w * 32 + lane];
+        const bool cand = active && t > 0 && ((t % P.check_every == 0 && sumO / (double)V < P.eps) || t == P.max_sweeps);
+        const double accE = half_sweep<N, 0, W1>(S, E, E, SV, O, P.lnk, hs, warp, lane, P.k2, active, cand, skipped);
+        hs = (hs + 1) % G::HSMOD;
+        // a4: gauge precision of the field after sweep t (R5), fixed summation order over the warps
+        if (warp < CW) sred[(rb * CW + warp) * 32 + lane] = accE;
+        __syncthreads();
+        double Ssum = sumO;
 #pragma unroll
         for (int w = 0; w < CW; ++w) Ssum += sred[(rb * CW + w) * 32 + lane];
         rb ^= 1;
@@ -463,6 +567,12 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
         dumpm = __ballot_sync(FULL, conv || maxed);
         need = dumpm;
     }
+#ifdef U1GF_TMA_PROF
+    __syncthreads();
+    if (blockIdx.x == 0 && tid == 0)
+        printf("prof N=%d: producer waits on empty %llu, warp 0 waits on full %llu, odd half-sweeps (warp 0) %llu, service %llu cycles\n", N,
+               g_prof[0], g_prof[1], g_prof[2], g_prof[3]);
+#endif
 }
 
 template <int N>
