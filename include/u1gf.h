@@ -96,9 +96,10 @@ int u1gf_relax_batch_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_sta
                           double* sig_host, double* g_canon_host);
 
 /* Kernel selection for u1gf_relax_batch on this handle: 0 = automatic (specialised resident kernel when one
- * exists for the extents; the streamed lane-per-start kernel for all-even lattices of 1024 sites and more and its
- * phased variant for lattices with an odd extent of 64 sites and more; else the generic one), 1 = force the generic
- * kernel, 2 = force the streamed / phased lane-per-start kernel.
+ * exists for the extents; the TMA-staged streamed kernel for 6^4 and 8^4; the streamed lane-per-start kernel for other
+ * all-even lattices of 1024 sites and more and its phased variant for lattices with an odd extent of 64 sites and more;
+ * else the generic one), 1 = force the generic kernel, 2 = force the streamed (plain loads) / phased lane-per-start
+ * kernel, 3 = force the TMA-staged streamed kernel (6^4, 8^4 only; other extents fall back to the generic kernel).
  * Results per start are the same copies either way; kernels may differ in the last bits of F and, rarely, by a
  * sweep (R14). */
 int u1gf_set_kernel(u1gf_orbit* o, int32_t which);
