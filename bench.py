@@ -293,7 +293,9 @@ def main():
     ap.add_argument("--config", type=int, default=4, help="BASELINE config id (1..5); 4 is the metric's workload")
     ap.add_argument("--orbit", type=int, default=0, help="orbit index inside the config")
     ap.add_argument("--starts", type=int, default=0, help="override the number of starts (debugging only)")
-    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 force the generic kernel")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic kernel, 2 streamed kernel with plain loads, 3 TMA-staged streamed kernel (u1gf_set_kernel)")
+    ap.add_argument("--eps", type=float, default=0.0, help="override eps (measurement only: with --max-sweeps, a fixed number of sweeps per start)")
+    ap.add_argument("--max-sweeps", type=int, default=0, help="override max_sweeps (measurement only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true", help="skip the `configs` section (BASELINE configs 1-3, 5)")
@@ -302,6 +304,8 @@ def main():
     ri = shard.rank_info_from_env()
     rank, world, local = ri.rank, ri.world, ri.local_rank
     conf, ob = workload(args.config, args.orbit, args.starts)
+    if args.eps or args.max_sweeps:
+        conf = dict(conf, eps=args.eps or conf["eps"], max_sweeps=args.max_sweeps or conf["max_sweeps"])
     ext, seed, n = ob["extents"], ob["seed"], ob["n_starts"]
     V, d = synth.volume(ext), len(ext)
     wl = f"config {args.config} orbit {args.orbit}: {conf['name']} {'x'.join(map(str, ext))} seed {seed}, {n} starts"
@@ -431,7 +435,7 @@ def main():
                               "only DMMA reaches (DESIGN.md section 7.1)") % A_D[d]})
 
     configs = None
-    if not args.no_all_configs and world == 1 and not args.starts:
+    if not args.no_all_configs and world == 1 and not args.starts and not args.eps and not args.max_sweeps:
         configs = {}
         csteps, cwarm = 2, 1
         for cid, oi in [(1, 0), (2, 0)] + [(5, k) for k in range(5)]:

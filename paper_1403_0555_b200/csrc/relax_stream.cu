@@ -428,7 +428,7 @@ __global__ void __launch_bounds__(kThreads, 1) relax_stream_kernel(const StreamP
 constexpr int kPhasedThreads = 128;
 constexpr int kPhasedWarps = kPhasedThreads / 32;
 
-template <int DIM, bool W1>
+template <int DIM, bool W1, bool SMEM>
 __global__ void __launch_bounds__(kPhasedThreads, 4) relax_phased_kernel(const StreamParams P) {
     constexpr unsigned FULL = 0xffffffffu;
     __shared__ double red[2][kPhasedWarps][5];
@@ -439,7 +439,9 @@ __global__ void __launch_bounds__(kPhasedThreads, 4) relax_phased_kernel(const S
     const OrbitDev& D = P.D;
     const int V = D.V;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    double2* const A = P.team_buf + (size_t)blockIdx.x * V * 32;   // [V][32 starts]
+    // the team's field [V][32 starts]: in shared memory when four teams fit an SM (V <= 110: 3^4), else in the workspace (L1)
+    extern __shared__ __align__(16) unsigned char phased_smem[];
+    double2* const A = SMEM ? reinterpret_cast<double2*>(phased_smem) : P.team_buf + (size_t)blockIdx.x * V * 32;
 
     bool active = false, maxed = false, skipped = false;
     int t = 0, rb = 0, fb = 0;
@@ -582,20 +584,22 @@ __global__ void __launch_bounds__(kPhasedThreads, 4) relax_phased_kernel(const S
     }
 }
 
-template <int DIM, bool W1>
+template <int DIM, bool W1, bool SMEM>
 int launch_phased_k(const u1gf_orbit* o, const RelaxArgs& a, StreamParams& P, cudaStream_t st) {
-    auto kern = relax_phased_kernel<DIM, W1>;
-    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 5);
+    auto kern = relax_phased_kernel<DIM, W1, SMEM>;
+    const size_t smem = SMEM ? (size_t)o->dev.V * 32 * sizeof(double2) : 0;
+    if (SMEM) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    else cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 5);
     int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kPhasedThreads, 0) != cudaSuccess) per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kPhasedThreads, smem) != cudaSuccess) per_sm = 0;
     unsigned long long teams = (unsigned long long)per_sm * (unsigned long long)o->sm_count;
     const unsigned long long batches = (a.n_starts + 31) / 32;
     if (teams > batches) teams = batches;
     if (teams > 4ull * (unsigned long long)o->sm_count) teams = 4ull * (unsigned long long)o->sm_count;   // workspace bound
     if (teams < 1) return fail(U1GF_ECUDA, "phased relaxation kernel does not fit on an SM");
-    const size_t bytes = 256 + (size_t)teams * (size_t)o->dev.V * 32 * sizeof(double2);
+    const size_t bytes = 256 + (SMEM ? 0 : (size_t)teams * (size_t)o->dev.V * 32 * sizeof(double2));
     U1GF_CUDA(cudaMemsetAsync(a.workspace, 0, bytes, st));
-    kern<<<(unsigned)teams, kPhasedThreads, 0, st>>>(P);
+    kern<<<(unsigned)teams, kPhasedThreads, smem, st>>>(P);
     U1GF_CUDA(cudaGetLastError());
     ++t_launches;
     return U1GF_OK;
@@ -653,7 +657,12 @@ int launch_phased(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st) {
     P.counter = (unsigned long long*)a.workspace;
     P.team_buf = (double2*)((char*)a.workspace + 256);
     P.D = o->dev;
-    return w1 ? launch_phased_k<DIM, true>(o, a, P, st) : launch_phased_k<DIM, false>(o, a, P, st);
+#ifndef U1GF_PHASED_SMEM_MAXV
+#define U1GF_PHASED_SMEM_MAXV 110   // 4 teams x V x 512 bytes within the shared memory of an SM
+#endif
+    if (o->dev.V <= U1GF_PHASED_SMEM_MAXV)
+        return w1 ? launch_phased_k<DIM, true, true>(o, a, P, st) : launch_phased_k<DIM, false, true>(o, a, P, st);
+    return w1 ? launch_phased_k<DIM, true, false>(o, a, P, st) : launch_phased_k<DIM, false, false>(o, a, P, st);
 }
 
 template <int DIM>

@@ -305,3 +305,52 @@ def test_full_size_first_region_counts_are_oracle_confirmed(b, oracle, cfg, orbi
     gpu_ids = _cpu(c["copy_id"])[ids]
     pairs = set(zip(gpu_ids.tolist(), oc["copy_id"].tolist()))
     assert len(pairs) == len(set(gpu_ids.tolist())) == len(set(oc["copy_id"].tolist()))
+
+
+# ------------------------------------------------------------------------------------------- TMA-staged streamed kernel
+@pytest.mark.parametrize("ext,seed", [((6, 6, 6, 6), 12), ((8, 8, 8, 8), 12)])
+def test_tma_kernel_options(b, oracle, ext, seed):
+    """relax_tma.cu on 6^4 / 8^4 against the oracle beyond the plain case of test_relax_matches_oracle: omega = 1 (its W1
+    instantiation) and 1.95, max_sweeps (the lanes that reach it keep their pre-update even values like the lanes that
+    converge: R5), check_every, start_ids / first_start / 64-bit seeds, a Gaussian orbit, and the same results from the
+    plain-load streamed kernel."""
+    V = int(np.prod(ext))
+    small = V > 2000
+    th = synth.uniform_links(ext, seed)
+    orbit = b.Orbit(ext, th)
+    assert orbit.kernel_name == "tma_stream_lane_per_start"
+
+    def gpu(n, sd=seed, **kw):
+        r = b.relax_batch(orbit, sd, n, want_g=True, **kw)
+        return {k: (_cpu(v) if v is not None and k != "workspace" else None) for k, v in r.items() if k != "workspace"}
+
+    def same(o, r):
+        assert (o["sweeps"] == r["sweeps"]).all() and (o["status"] == r["status"]).all()
+        assert np.abs(o["F_norm"] - r["F_norm"]).max() < TOL_F
+        assert np.abs(o["sig"] - r["sig"]).max() < TOL_G and np.abs(o["g_canon"] - r["g_canon"]).max() < TOL_G
+
+    n = 6 if small else 40
+    for omega in (1.0, 1.95):
+        same(oracle.relax(ext, th, seed, n, omega=omega, eps=1e-12, want_g=True), gpu(n, omega=omega, eps=1e-12))
+    for ms in (30, 90):    # none / some of the starts converge before the cap
+        o = oracle.relax(ext, th, seed, n, eps=1e-12, max_sweeps=ms, want_g=True)
+        r = gpu(n, eps=1e-12, max_sweeps=ms)
+        same(o, r)
+        assert (r["status"] & 1).any()
+    same(oracle.relax(ext, th, seed, n, eps=1e-11, check_every=3, want_g=True), gpu(n, eps=1e-11, check_every=3))
+    ids = np.array([5, 3, 2 ** 40 + 7, 3, 2 ** 63 + 11, 0], dtype=np.uint64)
+    sd = (9 << 32) | 1234567
+    same(oracle.relax(ext, th, sd, 0, start_ids=ids, eps=1e-11, want_g=True), gpu(0, sd=sd, start_ids=ids, eps=1e-11))
+    same(oracle.relax(ext, th, seed, 5, first_start=1000, eps=1e-11, want_g=True), gpu(5, first_start=1000, eps=1e-11))
+    # the plain-load streamed kernel gives the same copies and sweeps
+    r3 = gpu(n, eps=1e-12)
+    orbit.set_kernel(2)
+    r2 = gpu(n, eps=1e-12)
+    assert orbit.kernel_name == "stream_lane_per_start"
+    assert (r2["sweeps"] == r3["sweeps"]).all() and np.abs(r2["F_norm"] - r3["F_norm"]).max() < TOL_F
+    # Gaussian orbit + gauge transform (the shape of configs 2 / 4): few copies, short relaxations
+    thg = synth.gaussian_gauged_links(ext, 11, 0.8)
+    og = b.Orbit(ext, thg)
+    o = oracle.relax(ext, thg, 11, 70, want_g=True)
+    r = b.relax_batch(og, 11, 70, want_g=True)
+    same(o, {k: (_cpu(v) if v is not None and k != "workspace" else None) for k, v in r.items() if k != "workspace"})
