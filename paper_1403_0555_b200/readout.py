@@ -63,3 +63,18 @@ def format_bias_table(tab, top: int = 20) -> str:
                  f"mean sweeps {tab['sweeps_omega1']:.1f} vs {tab['sweeps_omega']:.1f}; "
                  f"mean x over starts {float((tab['x_paper'] * m1).sum() / n):.6f} vs {float((tab['x_paper'] * mw).sum() / n):.6f}")
     return "\n".join(lines)
+
+
+if __name__ == "__main__":
+    # python -m paper_1403_0555_b200.readout [config] [orbit] [n_starts]: the bias table of one BASELINE orbit as markdown
+    import sys
+    from . import synth
+    cfg = int(sys.argv[1]) if len(sys.argv) > 1 else 3
+    oi = int(sys.argv[2]) if len(sys.argv) > 2 else 0
+    conf = synth.CONFIGS[cfg]
+    ob = conf["orbits"][oi]
+    n = int(sys.argv[3]) if len(sys.argv) > 3 else ob["n_starts"]
+    orbit = b.Orbit(ob["extents"], synth.make_theta(ob))
+    tab = bias_table(orbit, ob["seed"], n, omega=conf["omega"], eps=conf["eps"], max_sweeps=conf["max_sweeps"])
+    print(f"config {cfg} orbit {oi}: {'x'.join(map(str, ob['extents']))} seed {ob['seed']}, {n} starts, eps {conf['eps']}, kernel {orbit.kernel_name}\n")
+    print(format_bias_table(tab, top=16))
