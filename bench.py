@@ -140,12 +140,12 @@ class Pipeline:
         nd = int(c["n_distinct"].item())                       # the only host read inside a step (8 bytes)
         self.fev[0].record()
         if self.store_g:
-            f = b.check_fp(self.orbit, self.out["g_canon"], index=c["rep"][:nd])
+            f = b.check_fp(self.orbit, self.out["g_canon"], index=c["rep"][:nd], want_steps=True)
             launches += b.last_launch_count()
         else:
             rr = b.relax_batch(self.orbit, self.seed, 0, start_ids=c["rep"][:nd] + self.first, want_g=True, **self.kw)
             launches += b.last_launch_count()
-            f = b.check_fp(self.orbit, rr["g_canon"])
+            f = b.check_fp(self.orbit, rr["g_canon"], want_steps=True)
             launches += b.last_launch_count()
         self.fev[1].record()
         # hot orbits (most starts are their own copy): write the fields of all starts in the first pass from now on,
@@ -177,11 +177,20 @@ class Pipeline:
             roof = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
                     "frac_at_48_bytes_moved": gbs * 1.5 / hbm_peak, "fp64_frac": fp64 / peak, "traffic": None}
         roof.update(kernel=name, kernel_ms=relax_ms, kernel_share_of_step=relax_ms / step_ms)
+        # a7: (2d+1) FP64 FMAs per site and Lanczos step (the mat-vec); first_region_ms also holds the
+        # re-relaxation of the representatives where the fields of all starts were not kept
+        steps = st["f"]["steps"]
+        lz_steps = int(steps.sum(dtype=torch.int64).item()) if steps is not None and nd else 0
+        lz_fma = float(lz_steps) * self.V * (2 * self.d + 1)
+        fp_roof = {"bound": "alu", "unit": "TFLOP/s", "lanczos_steps_mean": lz_steps / max(nd, 1),
+                   "algorithmic_fma_per_site_and_step": 2 * self.d + 1,
+                   "achieved": lz_fma * 2.0 / (max(fp_ms, 1e-6) * 1e-3) / 1e12, "peak": peak,
+                   "frac": lz_fma * 2.0 / (max(fp_ms, 1e-6) * 1e-3) / 1e12 / peak, "ms": fp_ms}
         return dict(workload=f"{'x'.join(map(str, self.ext))} seed {self.seed}, {self.n} starts", value=su / (step_ms * 1e-3),
                     ms_per_step=step_ms, relax_kernel_ms=relax_ms, first_region_ms=fp_ms,
                     first_region_path="fields of all starts kept, representatives by index" if "g_canon" in out and out["g_canon"] is not None
                     else "representatives re-relaxed",
-                    roofline=roof, converged_copies_per_s=conv / (step_ms * 1e-3), n_distinct=nd,
+                    roofline=roof, first_region_roofline=fp_roof, converged_copies_per_s=conv / (step_ms * 1e-3), n_distinct=nd,
                     n_in_first_region=int(st["f"]["n_in_region"].item()),
                     first_region_exceptions=exc_starts[:32], n_exceptions=len(exc_starts),
                     lanczos_unconverged=int((reg & 4).ne(0).sum().item()),
@@ -460,6 +469,7 @@ def main():
             "roofline": roofline, "cpu_baseline": cpu,
             "converged_copies_per_s": conv_all / (ms_per_step * 1e-3), "n_distinct": main_sum["n_distinct"],
             "n_in_first_region": main_sum["n_in_first_region"], "first_region_exceptions": main_sum["first_region_exceptions"],
+            "first_region_roofline": main_sum["first_region_roofline"],
             "mean_sweeps": sweeps_all / (n * world), "max_sweeps_seen": main_sum["max_sweeps_seen"], "configs": configs}
     print(json.dumps(line))
     if dist:

@@ -143,7 +143,9 @@ int u1gf_check_fp_host(const u1gf_orbit* o, uint64_t n_cfg, const double* g_host
  *   rep          dev [n] int64: rep[c] = position of the leader of copy c, c < n_distinct (rest undefined)
  *   multiplicity dev [n] int64: members of copy c
  *   hist         dev [nbins] int64 or NULL: histogram over nbins equal bins on [0,1] of F_norm[rep[c]] weighted by
- *                multiplicity[c] (PAPER.md:L167 uses width 1e-4)
+ *                multiplicity[c]: bin b holds F/(dV) in [b/nbins, (b+1)/nbins), values outside [0,1] go to the end bins.
+ *                The paper histograms the minimum value x = 1 - F/(dV) with bin width 1e-4: its bin j
+ *                is bin nbins-1-j here (mirror image; the half-open ends swap sides)
  *   workspace    dev scratch >= u1gf_count_workspace_bytes(n), 256-byte aligned
  * ------------------------------------------------------------------------------------------------------- */
 size_t u1gf_count_workspace_bytes(uint64_t n);

@@ -66,6 +66,12 @@ int u1gf_create_orbit(int d, const int32_t* extents, const double* theta_host, u
         }
         sgn[i] = bits;
     }
+    std::vector<uint8_t> fin(V);
+    for (int i = 0; i < V; ++i) {
+        bool last = true;
+        for (int mu = 0; mu < d; ++mu) last = last && phase[fwd[i * d + mu]] < phase[i] && phase[bwd[i * d + mu]] < phase[i];
+        fin[i] = last ? 1 : 0;
+    }
     // phases in order, empty ones dropped
     D.n_phases = 0;
     D.phase_off[0] = 0;
@@ -88,12 +94,12 @@ int u1gf_create_orbit(int d, const int32_t* extents, const double* theta_host, u
         o->U_host[2 * l + 1] = std::sin(theta_host[l]);
     }
 
-    // one device blob: U | fwd | bwd | order | sgn | lanes-layout links
+    // one device blob: U | fwd | bwd | order | sgn | fin | lanes-layout links | TMA-layout links
     auto align = [](size_t b) { return (b + 255) & ~(size_t)255; };
     const size_t bU = align((size_t)V * d * sizeof(double2)), bT = align((size_t)V * d * sizeof(int)),
                  bO = align((size_t)V * sizeof(int)), bS = align((size_t)V);
     const size_t bL = align(lanes_links_bytes(d, D.ext)), bM = align(tma_links_bytes(d, D.ext));
-    o->blob_bytes = bU + 2 * bT + bO + bS + bL + bM;
+    o->blob_bytes = bU + 2 * bT + bO + 2 * bS + bL + bM;
     cudaGetDevice(&o->device);
     cudaDeviceGetAttribute(&o->sm_count, cudaDevAttrMultiProcessorCount, o->device);
     cudaError_t e = cudaMalloc(&o->blob, o->blob_bytes);
@@ -120,6 +126,9 @@ int u1gf_create_orbit(int d, const int32_t* extents, const double* theta_host, u
     off += bO;
     std::memcpy(h + off, sgn.data(), (size_t)V);
     D.sgn = (const uint8_t*)(dptr + off);
+    off += bS;
+    std::memcpy(h + off, fin.data(), (size_t)V);
+    D.fin = (const uint8_t*)(dptr + off);
     off += bS;
     if (bL) {
         lanes_fill_links(d, D.ext, o->U_host.data(), (double2*)(h + off));

@@ -532,6 +532,10 @@ __global__ void __launch_bounds__(kPhasedThreads, 4) relax_phased_kernel(const S
         if (__ballot_sync(FULL, active) == 0) break;   // every warp holds the same lane states
 
         // ---------------------------------------------------------- one sweep: the phases of R3, in place
+        // accL: sum of Delta_i^2, taken right after the update, over the sites all of whose neighbours were updated
+        // before them in this sweep (D.fin): for these it is the Delta of the post-sweep field, so accL summed over the
+        // CTA is a LOWER BOUND of the gauge precision sum (with over-relaxation it is not zero: the update overshoots).
+        double accL = 0.0;
         for (int p = 0; p < D.n_phases; ++p) {
             const int q1 = D.phase_off[p + 1];
             for (int q = D.phase_off[p] + warp; q < q1; q += kPhasedWarps) {
@@ -551,32 +555,57 @@ __global__ void __launch_bounds__(kPhasedThreads, 4) relax_phased_kernel(const S
                     *own = gn;
                     skipped |= sk;
                 }
+                if (__ldg(D.fin + i)) {   // warp-uniform
+                    const double dl = fma(gn.y, wr, -gn.x * wi);
+                    accL = fma(dl, dl, accL);
+                }
             }
             __syncthreads();
         }
         if (active) ++t;
 
         // ---------------------------------------------------------- a4: gauge precision of the post-sweep field
-        double acc = 0.0;
-        for (int i = warp; i < V; i += kPhasedWarps) {
-            int jf[DIM], jb[DIM];
-#pragma unroll
-            for (int mu = 0; mu < DIM; ++mu) {
-                jf[mu] = __ldg(D.fwd + i * DIM + mu);
-                jb[mu] = __ldg(D.bwd + i * DIM + mu);
-            }
-            double wr, wi;
-            neighbour_sum<DIM>(D, A, i, jf, jb, lane, wr, wi);
-            const double2 g = A[(size_t)i * 32 + lane];
-            const double dl = fma(g.y, wr, -g.x * wi);   // Delta_i = Im(g_i conj w_i)
-            acc = fma(dl, dl, acc);
-        }
-        sred[rb][warp][lane] = acc;
+        // The full pass over the field (a second neighbour sum per site) is needed only if some lane that is tested at
+        // this sweep may pass: its lower bound is below 2 eps V (the factor 2 keeps rounding differences between the two
+        // sums out of the decision).  Otherwise no lane can stop and the pass is skipped -- the decision is unchanged.
+        sred[rb][warp][lane] = accL;
         __syncthreads();
-        double S = 0.0;
+        double Lsum = 0.0;
 #pragma unroll
-        for (int w = 0; w < kPhasedWarps; ++w) S += sred[rb][w][lane];
+        for (int w = 0; w < kPhasedWarps; ++w) Lsum += sred[rb][w][lane];
         rb ^= 1;
+        const bool tested = active && (t % P.check_every == 0);
+#ifdef U1GF_PHASED_ALWAYS_FULL   // knob: the full gauge-precision pass after every sweep (what the lower bound saves)
+        const bool may_pass = true;
+#elif defined(U1GF_PHASED_NEVER_FULL)   // ablation knob (wrong results: nothing ever converges)
+        const bool may_pass = false;
+#else
+        const bool may_pass = tested && !(Lsum / (double)V >= 2.0 * P.eps);
+#endif
+        double S = 0.0;
+        if (__syncthreads_or(may_pass ? 1 : 0)) {
+            double acc = 0.0;
+            for (int i = warp; i < V; i += kPhasedWarps) {
+                int jf[DIM], jb[DIM];
+#pragma unroll
+                for (int mu = 0; mu < DIM; ++mu) {
+                    jf[mu] = __ldg(D.fwd + i * DIM + mu);
+                    jb[mu] = __ldg(D.bwd + i * DIM + mu);
+                }
+                double wr, wi;
+                neighbour_sum<DIM>(D, A, i, jf, jb, lane, wr, wi);
+                const double2 g = A[(size_t)i * 32 + lane];
+                const double dl = fma(g.y, wr, -g.x * wi);   // Delta_i = Im(g_i conj w_i)
+                acc = fma(dl, dl, acc);
+            }
+            sred[rb][warp][lane] = acc;
+            __syncthreads();
+#pragma unroll
+            for (int w = 0; w < kPhasedWarps; ++w) S += sred[rb][w][lane];
+            rb ^= 1;
+        } else {
+            S = 2.0 * P.eps * (double)V;   // not below eps V for any tested lane
+        }
         const bool conv = active && (t % P.check_every == 0) && (S / (double)V < P.eps);
         maxed = active && !conv && t == P.max_sweeps;
         dumpm = __ballot_sync(FULL, conv || maxed);

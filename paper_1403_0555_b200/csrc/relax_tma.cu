@@ -58,7 +58,12 @@ struct TG {
 #define U1GF_TMA_SPW6 3
 #endif
     static constexpr int SPW = N == 8 ? U1GF_TMA_SPW8 : U1GF_TMA_SPW6;   // sites per consumer warp and step (knobs: 8^4: 4, 2, 1; 6^4: 3, 1)
-    static constexpr int CW = SITES / SPW;     // consumer warps (8^4: 8 x a half-line of 4 sites, 6^4: 6 x a half-line of 3)
+#ifndef U1GF_TMA_GRP6
+#define U1GF_TMA_GRP6 1
+#endif
+    static constexpr int NGRP = N >= 8 ? 1 : U1GF_TMA_GRP6;   // groups of consumer warps; group r works on the steps g = r (mod NGRP), so NGRP steps are in progress at a time
+    static constexpr int CWG = SITES / SPW;    // consumer warps of a group (8^4: 8 x a half-line of 4 sites, 6^4: 6 x a half-line of 3)
+    static constexpr int CW = CWG * NGRP;      // consumer warps
     static constexpr int THREADS = (CW + 1) * 32;   // + the producer warp
     static constexpr int V = N * N * N * N, HALF = V / 2;
     static constexpr int NS = N * N;           // steps per half-sweep
@@ -86,7 +91,7 @@ struct TG {
     static constexpr size_t off_pos = off_red + (size_t)2 * (CW + 1) * 5 * 8;
     static constexpr size_t off_skip = off_pos + 32 * 8;
     static constexpr size_t smem_bytes = off_skip + 32 * 4 + 16;
-    static_assert(SITES % SPW == 0 && N % 2 == 0, "geometry");
+    static_assert(SITES % SPW == 0 && N % 2 == 0 && (N * N) % (2 * NGRP) == 0 && ST > NGRP, "geometry");
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -270,7 +275,9 @@ __device__ __forceinline__ double half_sweep(const Smem<N>& S, const double2* sr
     // statements with a memory clobber, so the compiler keeps these loads behind them and is otherwise free to schedule
     auto lds = [&](unsigned off) { return *reinterpret_cast<const double2*>(S.base + off); };
     constexpr bool LINE = SPW == H;   // a warp owns a whole half-line: its H rows of the other parity serve all x0 neighbours
-    const int q0 = warp * SPW;        // first site of this warp inside a half-sheet, q = x1 * H + k
+    constexpr int NGRP = G::NGRP;
+    const int grp = warp / G::CWG;                // this warp works on the steps g = grp, grp + NGRP, ...
+    const int q0 = (warp % G::CWG) * SPW;         // first site of this warp inside a half-sheet, q = x1 * H + k
     const unsigned l16 = lane * 16;
     unsigned vF0[SPW][2], vB0[SPW][2], vF1[SPW], vB1[SPW], vQ[SPW];   // byte offsets inside a half-sheet (+ the lane's 16 bytes)
     unsigned vRow[LINE ? H : 1];
@@ -292,16 +299,29 @@ __device__ __forceinline__ double half_sweep(const Smem<N>& S, const double2* sr
         if (LINE) vRow[LINE ? j : 0] = vQ[j];
     }
     double2 own[SPW], nxt[SPW];
-    const double2* psrc = src + (size_t)q0 * 32 + lane;
-    double2* pdst = dst + (size_t)q0 * 32 + lane;
+    const double2* psrc = src + ((size_t)grp * SITES + q0) * 32 + lane;
+    double2* pdst = dst + ((size_t)grp * SITES + q0) * 32 + lane;
 #pragma unroll
     for (int j = 0; j < SPW; ++j) own[j] = __ldcs(psrc + j * 32);
     // ring positions of step 0: window fetch of the x2-1 half-sheet (slot, phase parity), stage (index, phase parity)
     unsigned sDn = wl0 % RW, pDn = (wl0 / RW) & 1u, st = step0 % ST, pst = (step0 / ST) & 1u;
     int x2 = 0, sp = 0;   // sp = (x2 + x3) & 1
+    // the window advances by one fetch inside a layer and by three at a layer boundary (N + 2 fetches per layer)
+    auto advance = [&]() {
+        if (++st == ST) st = 0, pst ^= 1u;
+        if (++x2 == N) {
+            x2 = 0;   // x2: N-1 -> 0 and x3 + 1: the sheet parity stays
+            sDn += 3;
+        } else {
+            sp ^= 1;
+            sDn += 1;
+        }
+        if (sDn >= RW) sDn -= RW, pDn ^= 1u;
+    };
+    for (int r = 0; r < grp; ++r) advance();
     auto step = [&](int g, double2 (&own)[SPW], double2 (&nxt)[SPW]) {
-        psrc += SITES * 32;
-        if (g + 1 < NS) {
+        psrc += NGRP * SITES * 32;
+        if (g + NGRP < NS) {
 #pragma unroll
             for (int j = 0; j < SPW; ++j) nxt[j] = __ldcs(psrc + j * 32);
         }
@@ -310,7 +330,7 @@ __device__ __forceinline__ double half_sweep(const Smem<N>& S, const double2* sr
         unsigned sUp = sC + 1, pUp = pC;
         if (sUp == RW) sUp = 0, pUp ^= 1u;
         PROF_T0();
-        if (x2 == 0) {   // first step of a layer: all three half-sheets are new; later ones were waited for as C / Up
+        if (NGRP > 1 || x2 == 0) {   // first step of a layer: all three half-sheets are new; later ones were waited for as C / Up
             mbar_wait(S.fullW + sDn * 8, pDn);
             mbar_wait(S.fullW + sC * 8, pC);
         }
@@ -378,23 +398,15 @@ __device__ __forceinline__ double half_sweep(const Smem<N>& S, const double2* sr
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(S.empty + st * 8);   // this warp no longer reads the buffers of step g
-        pdst += SITES * 32;
-        // next step: the window advances by one fetch inside a layer and by three at a layer boundary (N + 2 fetches per layer)
-        if (++st == ST) st = 0, pst ^= 1u;
-        if (++x2 == N) {
-            x2 = 0;   // x2: N-1 -> 0 and x3 + 1: the sheet parity stays
-            sDn += 3;
-        } else {
-            sp ^= 1;
-            sDn += 1;
-        }
-        if (sDn >= RW) sDn -= RW, pDn ^= 1u;
+        pdst += NGRP * SITES * 32;
+#pragma unroll
+        for (int r = 0; r < NGRP; ++r) advance();
     };
     // two steps per iteration: the rows fetched for the next step land in the other register set (no copies, so the
     // load has a whole step to arrive)
-    for (int g = 0; g < NS; g += 2) {
+    for (int g = grp; g < NS; g += 2 * NGRP) {
         step(g, own, nxt);
-        step(g + 1, nxt, own);
+        step(g + NGRP, nxt, own);
     }
     if (PAR == 1 && !commit) acc = 0.0;
     return acc;
@@ -436,7 +448,7 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
         for (int s = 0; s < G::RW; ++s) mbar_init(S.fullW + s * 8, 1);
         for (int s = 0; s < G::ST; ++s) {
             mbar_init(S.fullS + s * 8, 1);
-            mbar_init(S.empty + s * 8, CW);
+            mbar_init(S.empty + s * 8, G::CWG);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }

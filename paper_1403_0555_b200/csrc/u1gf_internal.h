@@ -92,6 +92,8 @@ struct OrbitDev {
     const int* bwd;                 // [V*d] index of i-mu
     const int* order;               // [V] sites sorted by (phase, index)
     const uint8_t* sgn;             // [V] signature sign bits: bit k = a_{k,i} is +1, bit 4+k = b_{k,i} is +1
+    const uint8_t* fin;             // [V] 1: every neighbour of the site is updated before it in a sweep, so its Delta right
+                                    //     after its own update is its Delta on the field after the sweep (phased kernel, R5)
 };
 
 }  // namespace u1gf
