@@ -438,6 +438,9 @@ def main():
                      if roofline["bound"] == "alu" else None,
                      "dfma_rate_3_register_operands": rate_rrr * 2.0 / 1e12, "dfma_rate_complex_mac": rate_mac * 2.0 / 1e12,
                      "hbm_peak_source": hbm_how,
+                     "traffic_note": ("traffic is null: the relaxation state never leaves the SM; ncu on 262144 starts of this orbit "
+                                      "(profiles/r02_ncu_summaries.md): 13.6 MB DRAM read + 1.96 GB written per launch = 7.5 KB per start "
+                                      "(start / dump rings and outputs) against 1.2e4 site updates per start"),
                      "note": ("achieved = site-updates x (8d+16 = %d algorithmic FP64 instructions) x 2 flop / kernel time "
                               "(CUDA events on the launching stream around u1gf_relax_batch); frac = against the DFMA "
                               "microbenchmark, frac_of_fp64_pipe / frac_of_dmma_rate = against 64 lanes x SMs x clock, which "
