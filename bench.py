@@ -220,8 +220,9 @@ def time_pipeline(p, torch, flush, steps, warmup, barrier=None):
         barrier()
     else:
         torch.cuda.synchronize()
-    total_ms = sum(a.elapsed_time(z) for a, z in ev)
-    return total_ms, float(np.mean(relax_ms)), float(np.mean(fp_ms))
+    per_step = [a.elapsed_time(z) for a, z in ev]
+    time_pipeline.last_per_step = per_step      # the `configs` section reports the median step (few repetitions, one hiccup would show)
+    return sum(per_step), float(np.mean(relax_ms)), float(np.mean(fp_ms))
 
 
 def ensemble_config3(b, torch, flush, steps, warmup, peak_dfma, sm_clock_mhz, sms):
@@ -273,7 +274,7 @@ def ensemble_config3(b, torch, flush, steps, warmup, peak_dfma, sm_clock_mhz, sm
     r = st["r"]
     sweeps = r["sweeps"].sum(dim=1, dtype=torch.int64).cpu().tolist()
     su = float(V) * float(sum(sweeps))
-    step_ms, relax_ms = float(np.mean(ms)), float(np.mean(rms))
+    step_ms, relax_ms = float(np.median(ms)), float(np.median(rms))
     n_in = [int(st["f"][k][0]["n_in_region"].item()) for k in range(len(seeds))]
     exc = {int(seeds[k]): st["f"][k][1][torch.nonzero(st["f"][k][0]["region"] != 1).flatten()].cpu().tolist() for k in range(len(seeds))}
     fp64 = su * A_D[3] * 2.0 / (relax_ms * 1e-3) / 1e12
@@ -449,13 +450,13 @@ def main():
     configs = None
     if not args.no_all_configs and world == 1 and not args.starts and not args.eps and not args.max_sweeps:
         configs = {}
-        csteps, cwarm = 2, 1
+        csteps, cwarm = 3, 1
         for cid, oi in [(1, 0), (2, 0)] + [(5, k) for k in range(5)]:
             c2, o2 = workload(cid, oi, 0)
             p2 = Pipeline(b, torch, c2, o2, 0)
             t_ms, r_ms, f_ms = time_pipeline(p2, torch, flush, csteps, cwarm + (1 if cid == 5 and oi >= 2 else 0))
-            s2, _, _, _ = p2.summary(r_ms, f_ms, t_ms / csteps, peak_dfma, sm_clock, sms, hbm_peak)
-            s2.update(steps=csteps, warmup=cwarm)
+            s2, _, _, _ = p2.summary(r_ms, f_ms, float(np.median(time_pipeline.last_per_step)), peak_dfma, sm_clock, sms, hbm_peak)
+            s2.update(steps=csteps, warmup=cwarm, ms_per_step_is="median of the timed steps")
             configs[f"cfg{cid}_{'x'.join(map(str, o2['extents']))}"] = s2
             del p2
             torch.cuda.empty_cache()
