@@ -306,6 +306,7 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic kernel, 2 streamed kernel with plain loads, 3 TMA-staged streamed kernel (u1gf_set_kernel)")
     ap.add_argument("--eps", type=float, default=0.0, help="override eps (measurement only: with --max-sweeps, a fixed number of sweeps per start)")
     ap.add_argument("--max-sweeps", type=int, default=0, help="override max_sweeps (measurement only)")
+    ap.add_argument("--merge-tables", action="store_true", help="run the copy-table merge of the multi-GPU path at N = 1 too")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true", help="skip the `configs` section (BASELINE configs 1-3, 5)")
@@ -391,6 +392,18 @@ def main():
     site_updates = float(V) * float(sweeps_all)              # per step, all ranks
     value = site_updates / (ms_per_step * 1e-3)
 
+    # N > 1: the ranks' copy tables merged into the job's table, outside the timed region: all-gather of
+    # {F, signature, global first start, multiplicity} of the representatives, then u1gf_merge_copy_tables on every rank
+    n_distinct_global = None
+    if world > 1 or args.merge_tables:
+        st = pipe.state
+        nd = st["n_distinct"]
+        rep = st["c"]["rep"][:nd]
+        F, S, fs, mu, offs = shard.gather_copy_tables(pipe.out["F_norm"][rep], pipe.out["sig"][rep], rep + first,
+                                                      st["c"]["multiplicity"][:nd], dist)
+        mg = b.merge_copy_tables(F, S, fs, mu)
+        n_distinct_global = int(mg["n_merged"].item())
+
     # e2e: the whole path through u1gf_pipeline_host: link angles in (u1gf_create_orbit), host result arrays out
     e2e = None
     if not args.no_e2e:
@@ -472,6 +485,7 @@ def main():
             "gpu_launches_note": "kernels of libu1gf.so per step, counted by the library; CUB's sort/scan launches inside u1gf_count_copies are extra",
             "roofline": roofline, "cpu_baseline": cpu,
             "converged_copies_per_s": conv_all / (ms_per_step * 1e-3), "n_distinct": main_sum["n_distinct"],
+            "n_distinct_all_ranks_merged": n_distinct_global,
             "n_in_first_region": main_sum["n_in_first_region"], "first_region_exceptions": main_sum["first_region_exceptions"],
             "first_region_roofline": main_sum["first_region_roofline"],
             "mean_sweeps": sweeps_all / (n * world), "max_sweeps_seen": main_sum["max_sweeps_seen"], "configs": configs}
