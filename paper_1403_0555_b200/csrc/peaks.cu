@@ -233,8 +233,10 @@ int u1gf_measure_fp64_peak(double ms, double* dfma_per_s, void* cuda_stream) {
     const int threads = 512, blocks = sms * 4;
     U1GF_CUDA(cudaMalloc(&scratch, (size_t)threads * blocks * sizeof(double)));
     cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        cudaFree(scratch);
+        return fail(U1GF_ECUDA, "cudaEventCreate failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
     const int iters = 4096;
     const double per_launch = (double)threads * blocks * (double)iters * 4.0 * kChains;
     double best = 0.0, spent = 0.0;
@@ -291,8 +293,10 @@ int u1gf_measure_fp64_rate(int32_t pattern, double ms, double* dfma_per_s, void*
         }
     };
     cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        cudaFree(scratch);
+        return fail(U1GF_ECUDA, "cudaEventCreate failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
     // thread-level FMAs per launch: 32 per iteration, except the DMMA stream (32 instructions x 8 FMAs)
     const double per_launch = (double)threads * blocks * (double)iters * 32.0 * (pattern == 6 ? 8.0 : 1.0);
     double best = 0.0, spent = 0.0;
@@ -336,8 +340,10 @@ int u1gf_measure_smem_peak(double ms, double* bytes_per_s, void* cuda_stream) {
     U1GF_CUDA(cudaFuncSetAttribute(lds_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     U1GF_CUDA(cudaMalloc(&scratch, (size_t)threads * blocks * sizeof(unsigned)));
     cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        cudaFree(scratch);
+        return fail(U1GF_ECUDA, "cudaEventCreate failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
     const int iters = 4096;
     const double per_launch = (double)threads * blocks * (double)iters * 8.0 * 16.0;
     double best = 0.0, spent = 0.0;
@@ -382,8 +388,10 @@ int u1gf_measure_smem_rate(int32_t mix, double ms, double* instr_per_s, void* cu
     unsigned* scratch = nullptr;
     U1GF_CUDA(cudaMalloc(&scratch, (size_t)threads * sizeof(unsigned)));
     cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        cudaFree(scratch);
+        return fail(U1GF_ECUDA, "cudaEventCreate failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
     const double per_launch = (double)(threads / 32) * blocks * (double)iters * 8.0 * per_site;   // warp-level instructions
     double best = 0.0, spent = 0.0;
     kern<<<blocks, threads, smem, st>>>(scratch, 16);
@@ -442,8 +450,10 @@ int u1gf_measure_dsmem_rate(int32_t cluster_size, int32_t remote, double ms, dou
     double* scratch = nullptr;
     U1GF_CUDA(cudaMalloc(&scratch, 64));
     cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        cudaFree(scratch);
+        return fail(U1GF_ECUDA, "cudaEventCreate failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
     const int iters = 4000;
     const double per_cta = (double)iters * 8.0 * 512.0 * 16.0;   // 16 warps x 8 loads x 512 bytes per iteration
     double best = 0.0, spent = 0.0;
