@@ -10,9 +10,10 @@
 // with conflict-free LDS.128.  The data in flight sits in shared memory (about 100 KB per SM), not in registers.
 //
 // Layout of a team's field (workspace): three arrays O (odd sites), E (even sites) and SV (the pre-update even values
-// of the lanes that may stop at this sweep, see below), each [sheet = x3*N + x2][x1][k][32 starts] double2, where the half-line (x1, x2, x3) of parity p holds
-// the sites x0 = 2k + ((p + x1 + x2 + x3) & 1), k = 0 .. N/2-1.  A "half-sheet" (all x0, x1 of one parity at fixed
-// x2, x3) is one contiguous block of N * N/2 rows = 16 KB at N = 8, 9 KB at N = 6: the unit of a bulk copy.
+// of the lanes that may stop at this sweep, see the kernel), each [sheet = x3*N + x2][x1][k][32 starts] double2, where
+// the half-line (x1, x2, x3) of parity p holds the sites x0 = 2k + ((p + x1 + x2 + x3) & 1), k = 0 .. N/2-1.  A
+// "half-sheet" (all x0, x1 of one parity at fixed x2, x3) is one contiguous block of N * N/2 rows = 16 KB at N = 8,
+// 9 KB at N = 6: the unit of a bulk copy.
 //
 // A half-sweep walks the sheets in order (x3 outer, x2 inner), one step per sheet.  For the sites of parity p in sheet
 // (x2, x3) the neighbours along x0 and x1 are in the other-parity half-sheet (x2, x3), those along x2 in the
@@ -20,10 +21,10 @@
 // once per layer (N + 2 fetches for N steps) -- and those along x3 in the half-sheets (x2, x3 -+ 1), fetched per step
 // into a ring of ST stages together with the step's links ([site][8] double2: U_{i,mu}, U_{i-mu,mu}).  Per site
 // update: 16 B (window) * (N+2)/N + 32 B (x3 neighbours) + 16 B own row read + 16 B written = 84 B between L2 and
-// the SM, of which the 48 B that are not re-reads come from HBM (the x3 re-reads hit L2: two layers of a team's rows
-// are 2 x 3 x 128 KB at 8^4, 114 MB over 148 teams; own rows carry streaming hints).  The own row of a site is
-// private to the thread that updates it (same warp, same lane every sweep): it is read by a plain coalesced load one
-// step ahead and written back from registers.
+// the SM; at 8^4 the 48 B that are not re-reads come from HBM (the x3 re-reads hit L2; own rows carry streaming
+// hints), at 6^4 the 96 MB that 148 teams cycle through stay in L2.  The own row of a site is private to the thread
+// that updates it (same warp, same lane every sweep): it is read by a plain coalesced load one step ahead and written
+// back from registers.  Measured bounds and what was tried: DESIGN.md section 7.4, profiles/r02_ablations.md.
 //
 // Arithmetic of a site update, stop rule (R5), lane-level refill and finalisation are those of relax_stream.cu.
 #include "u1gf_internal.h"
