@@ -32,7 +32,10 @@ __device__ __forceinline__ double block_sum(double a, double (*red)[32], int& bu
     if (lane == 0) red[buf][warp] = a;
     __syncthreads();
     double s = 0.0;
-    for (int w = 0; w < nw; ++w) s += red[buf][w];
+    if (nw == 2) s = red[buf][0] + red[buf][1];   // the small lattices: one or two warps per configuration
+    else if (nw == 1) s = red[buf][0];
+    else
+        for (int w = 0; w < nw; ++w) s += red[buf][w];
     buf ^= 1;
     return s;
 }
@@ -131,9 +134,17 @@ __device__ __forceinline__ void block_sum2(double& a, double& b, double (*red2)[
     }
     __syncthreads();
     double sa = 0.0, sb = 0.0;
-    for (int w = 0; w < nw; ++w) {
-        sa += red2[buf][w][0];
-        sb += red2[buf][w][1];
+    if (nw == 2) {
+        sa = red2[buf][0][0] + red2[buf][1][0];
+        sb = red2[buf][0][1] + red2[buf][1][1];
+    } else if (nw == 1) {
+        sa = red2[buf][0][0];
+        sb = red2[buf][0][1];
+    } else {
+        for (int w = 0; w < nw; ++w) {
+            sa += red2[buf][w][0];
+            sb += red2[buf][w][1];
+        }
     }
     a = sa;
     b = sb;
