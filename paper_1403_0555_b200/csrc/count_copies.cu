@@ -112,9 +112,19 @@ __global__ void __launch_bounds__(256) elect_kernel(const double* __restrict__ s
         unsigned* cur = (round & 1) ? w.run_min1 : w.run_min0;
         unsigned* nxt = (round & 1) ? w.run_min0 : w.run_min1;
         if (t0 == 0) rem[(round + 1) & 1] = 0;
-        for (unsigned j = t0; j < n_conv; j += stride) {
-            const unsigned p = w.pos_out[j];
-            if (w.leader_of[p] < 0) atomicMin(&cur[w.run_id[j] - 1], p);
+        // candidates: the smallest position among the unassigned records of each run.  Sorted order puts the records of a
+        // run next to each other, so the lanes of a warp mostly share a run: one atomic per run and warp (2^22 starts
+        // in 5 copies would otherwise send 4 million atomics to 5 addresses)
+        for (unsigned jb = t0 - (threadIdx.x & 31); jb < n_conv; jb += stride) {   // warp-uniform trip count
+            const unsigned j = jb + (threadIdx.x & 31);
+            unsigned r = kNone, p = kNone;
+            if (j < n_conv) {
+                p = w.pos_out[j];
+                if (w.leader_of[p] < 0) r = w.run_id[j] - 1;
+            }
+            const unsigned peers = __match_any_sync(0xffffffffu, r);
+            const unsigned pmin = __reduce_min_sync(peers, p);
+            if (r != kNone && (threadIdx.x & 31) == (unsigned)(__ffs(peers) - 1)) atomicMin(&cur[r], pmin);
         }
         grid.sync();
         bool left = false;
