@@ -25,12 +25,24 @@ struct FpParams {
     const int64_t* index;   // configuration k is g[index[k]] (NULL: g[k])
 };
 
+// ASYNC kernels carry one extra warp (the last) that runs the Ritz tests: barrier 1 joins the compute warps, barrier 2
+// the whole CTA (rendezvous with the Ritz warp); the other kernels use the ordinary CTA barrier.
+template <bool ASYNC>
+__device__ __forceinline__ void compute_barrier() {
+    if (ASYNC) asm volatile("bar.sync 1, %0;" ::"r"(blockDim.x - 32) : "memory");
+    else __syncthreads();
+}
+__device__ __forceinline__ void cta_barrier() { asm volatile("bar.sync 2, %0;" ::"r"(blockDim.x) : "memory"); }
+template <bool ASYNC>
+__device__ __forceinline__ int compute_warps() { return ASYNC ? (int)((blockDim.x - 32) >> 5) : (int)((blockDim.x + 31) >> 5); }
+
+template <bool ASYNC>
 __device__ __forceinline__ double block_sum(double a, double (*red)[32], int& buf) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) a += __shfl_down_sync(0xffffffffu, a, o);
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = compute_warps<ASYNC>();
     if (lane == 0) red[buf][warp] = a;
-    __syncthreads();
+    compute_barrier<ASYNC>();
     double s = 0.0;
     if (nw == 2) s = red[buf][0] + red[buf][1];   // the small lattices: one or two warps per configuration
     else if (nw == 1) s = red[buf][0];
@@ -121,18 +133,19 @@ __device__ double last_component(const double* alpha, const double* beta, const 
 }
 
 // Sum of two values over the CTA, same result in every thread, fixed tree (see block_sum).
+template <bool ASYNC>
 __device__ __forceinline__ void block_sum2(double& a, double& b, double (*red2)[32][2], int& buf) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         a += __shfl_down_sync(0xffffffffu, a, o);
         b += __shfl_down_sync(0xffffffffu, b, o);
     }
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = compute_warps<ASYNC>();
     if (lane == 0) {
         red2[buf][warp][0] = a;
         red2[buf][warp][1] = b;
     }
-    __syncthreads();
+    compute_barrier<ASYNC>();
     double sa = 0.0, sb = 0.0;
     if (nw == 2) {
         sa = red2[buf][0][0] + red2[buf][1][0];
@@ -151,28 +164,113 @@ __device__ __forceinline__ void block_sum2(double& a, double& b, double (*red2)[
     buf ^= 1;
 }
 
-// One CTA per configuration, every thread owns up to SPT sites (i = tid, tid + T, ...).  The neighbour indices of a
-// thread's sites are the same for every configuration and every step: they are read once into registers (16-bit,
+// History of the Ritz tests of one configuration (registers of the warp that runs them) and one test.
+struct RitzState {
+    double lam, lam_hi, res_prev, last_drop;
+    int k_prev, n_checks;
+    bool have_drop;
+    __device__ void reset(int dim) {
+        lam = 0.0; lam_hi = 4.0 * dim + 1.0; res_prev = 0.0; last_drop = 0.0;
+        k_prev = 0; n_checks = 0; have_drop = false;
+    }
+};
+
+// Test of T_k by one warp (all 32 lanes call this): smallest Ritz value `l`, residual bound `res`, and `step`, the
+// distance from k to where the bound, which falls geometrically, is expected to cross 1e-10.  final: refine the Ritz
+// value whatever the residual (breakdown or step cap).
+template <int DIM>
+__device__ void ritz_test(RitzState& R, const double* alpha, const double* beta, const double* beta2, const double* ibeta,
+                          int k, bool breakdown, bool final, double& l, double& res, int& step) {
+    // Ritz values decrease with k (interlacing): the new one lies below the last; a lower end a few times the last
+    // decrease below it is tried first (one Sturm count says whether it holds)
+    double lo_try = -(4.0 * DIM + 1.0);
+    if (R.have_drop) {
+        const double cand = R.lam - 8.0 * R.last_drop - 1e-9;
+        if (sturm_count(alpha, beta2, k, cand) == 0) lo_try = cand;
+    }
+    // the Ritz value to 1e-11 is enough to follow the residual; it is refined to 2e-14 once the test passes
+    l = smallest_ritz(alpha, beta2, k, lo_try, R.lam_hi, 1e-11);
+    res = breakdown ? 0.0 : beta[k - 1] * last_component(alpha, beta, ibeta, k, l - 1e-13);
+    if (final || res < 1e-10) l = smallest_ritz(alpha, beta2, k, l - 2e-11 * fmax(1.0, fabs(l)), l + 2e-11 * fmax(1.0, fabs(l)), 2e-14);
+    if (R.n_checks > 0) {
+        R.last_drop = fmax(R.lam - l, 0.0);
+        R.have_drop = true;
+    }
+    R.lam = l;
+    R.lam_hi = l + 1e-9;
+    step = max(4, k / 4);
+    if (R.n_checks > 0 && res > 0.0 && res < R.res_prev) {   // (a measured decay may carry the next test up to k/2 ahead)
+        const double per_step = log(R.res_prev / res) / (double)(k - R.k_prev);
+        step = max(3, min(max(4, k / 2), (int)(0.9 * log(res / 1e-10) / per_step) + 1));
+    }
+    R.res_prev = res;
+    R.k_prev = k;
+    ++R.n_checks;
+}
+
+// Mailbox between the compute warps and the Ritz warp of an ASYNC kernel (shared memory).  A rendezvous is two CTA
+// barriers: before the first the compute side has written the command and the Ritz warp the verdict of its last test;
+// between the two each side reads the other's fields into registers; after the second both may write again.
+struct RitzMail {
+    int cmd_k;       // > 0: test T_k; 0: nothing (the compute side only wants the verdict); < 0: leave
+    int cmd_flags;   // 1: first test of a configuration (forget the history); 2: final; 4: breakdown
+    int v_k, v_step; // verdict: the k it belongs to; predicted distance to the crossing
+    double v_lam, v_res;
+};
+
+// One CTA per configuration, every compute thread owns up to SPT sites (i = tid, tid + T, ...).  The neighbour indices
+// of a thread's sites are the same for every configuration and every step: they are read once into registers (16-bit,
 // V <= 8192) instead of 2 DIM index loads per site and mat-vec.  Per Lanczos step: the mat-vec with <w, v1> (one
 // reduction), w -= alpha v1 with the mean of w and its norm without the mean, sum w^2 - V mean^2, in ONE reduction, then
 // the scaled vector -- three barriers per step.
-template <int DIM, int SPT, int MAXT>
-__global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) lanczos_kernel(const OrbitDev D, const FpParams P) {
+// The Ritz test is serial work of one warp.  Small lattices (several CTAs per SM): warp 0 runs it while the others wait;
+// other configurations fill the SM.  ASYNC (the large lattices, one or two CTAs per SM, where nothing else fills the
+// gap): an extra warp runs the test concurrently with the following Lanczos steps, which only append to the coefficient
+// arrays; at a test point the compute warps hand over T_k and pick up the verdict of the PREVIOUS test.  A configuration
+// ends at the first test that passes, in test order; which tests are made depends only on the data, never on timing, so
+// lambda_1, region and step count are reproducible; the few steps taken after the passing test are discarded.
+template <int DIM, int SPT, int MAXT, bool ASYNC>
+__global__ void __launch_bounds__(MAXT + (ASYNC ? 32 : 0), MAXT <= 256 ? 2 : 1) lanczos_kernel(const OrbitDev D, const FpParams P) {
     extern __shared__ double sm[];
-    const int V = D.V, tid = threadIdx.x, T = blockDim.x;
+    const int V = D.V, tid = threadIdx.x, T = blockDim.x - (ASYNC ? 32 : 0);
     double* c = sm;                 // [DIM][V]
     double* va = c + (size_t)V * DIM;  // [V]
     double* vb = va + V;            // [V]
     __shared__ double red[2][32];
     __shared__ double red2[2][32][2];
+    __shared__ RitzMail mail;
     const int kcap = min(V - 1, kMaxK);
     double* alpha = vb + V;   // Lanczos coefficients [4][kcap], behind the vectors in dynamic shared memory
     double* beta = alpha + kcap;
     double* beta2 = beta + kcap;
     double* ibeta = beta2 + kcap;
-    __shared__ double s_lam, s_res;
     int buf = 0, buf2 = 0;
     const int kmax = kcap;
+    RitzState R;
+    R.reset(DIM);
+
+    if (ASYNC && tid >= T) {
+        // ------------------------------------------------------------------ the Ritz warp
+        for (;;) {
+            cta_barrier();
+            const int k = mail.cmd_k, flags = mail.cmd_flags;
+            cta_barrier();
+            if (k < 0) break;
+            if (k == 0) continue;
+            if (flags & 1) R.reset(DIM);
+            double l, res;
+            int step;
+            ritz_test<DIM>(R, alpha, beta, beta2, ibeta, k, (flags & 4) != 0, (flags & 2) != 0, l, res, step);
+            if ((tid & 31) == 0) {
+                mail.v_k = k;
+                mail.v_step = step;
+                mail.v_lam = l;
+                mail.v_res = res;
+            }
+            __syncwarp();
+        }
+        return;
+    }
 
     unsigned short nf[SPT][DIM], nb[SPT][DIM];
 #pragma unroll
@@ -184,10 +282,23 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) lanczos_kernel(cons
             nb[s][mu] = i < V ? (unsigned short)__ldg(D.bwd + i * DIM + mu) : (unsigned short)0;
         }
     }
+    // ASYNC: hand a command to the Ritz warp and pick up its last verdict
+    auto rendezvous = [&](int k, int flags, int& vk, int& vstep, double& vlam, double& vres) {
+        if (tid == 0) {
+            mail.cmd_k = k;
+            mail.cmd_flags = flags;
+        }
+        cta_barrier();
+        vk = mail.v_k;
+        vstep = mail.v_step;
+        vlam = mail.v_lam;
+        vres = mail.v_res;
+        cta_barrier();
+    };
 
     for (unsigned long long cfg = blockIdx.x; cfg < P.n_cfg; cfg += gridDim.x) {
         const double2* g = P.g + (P.index ? (unsigned long long)P.index[cfg] : cfg) * (unsigned long long)V;
-        __syncthreads();
+        compute_barrier<ASYNC>();
         // weights c_{i,mu} = Re(g_i U_{i,mu} conj g_{i+mu}), stored [mu][V]: consecutive lanes, consecutive banks
         double s1 = 0.0;
 #pragma unroll
@@ -208,7 +319,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) lanczos_kernel(cons
                 s1 += x;
             }
         }
-        s1 = block_sum(s1, red, buf);
+        s1 = block_sum<ASYNC>(s1, red, buf);
         const double mean0 = s1 / (double)V;
         double s2 = 0.0;
 #pragma unroll
@@ -221,22 +332,21 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) lanczos_kernel(cons
                 vb[i] = 0.0;
             }
         }
-        s2 = block_sum(s2, red, buf);
+        s2 = block_sum<ASYNC>(s2, red, buf);
         const double inv0 = rsqrt(s2);
 #pragma unroll
         for (int s = 0; s < SPT; ++s) {
             const int i = tid + s * T;
             if (i < V) va[i] *= inv0;
         }
-        __syncthreads();
+        compute_barrier<ASYNC>();
 
         double* v1 = va;  // current Lanczos vector
         double* v0 = vb;  // previous one; overwritten by the new direction
-        double beta_prev = 0.0, lam = 0.0, lam_hi = 4.0 * DIM + 1.0;
-        int k = 0, next_check = 16, k_prev = 0, n_checks = 0;
-        double res_prev = 0.0, last_drop = 0.0;
-        bool have_drop = false;
+        double beta_prev = 0.0, lam = 0.0;
+        int k = 0, next_check = 16, n_handed = 0, k_out = 0;
         bool done = false, unconverged = false;
+        if (!ASYNC) R.reset(DIM);
         while (!done) {
             // w = M v1 - beta_prev v0 (kept in registers), alpha = <w, v1>
             double w[SPT], vi[SPT], a = 0.0;
@@ -258,7 +368,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) lanczos_kernel(cons
                     a = fma(w[s], vi[s], a);
                 }
             }
-            a = block_sum(a, red, buf);
+            a = block_sum<ASYNC>(a, red, buf);
             // w -= alpha v1; its mean (the constant mode, taken out every step) and its norm without the mean
             double sw = 0.0, sww = 0.0;
 #pragma unroll
@@ -267,7 +377,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) lanczos_kernel(cons
                 sw += w[s];
                 sww = fma(w[s], w[s], sww);
             }
-            block_sum2(sw, sww, red2, buf2);
+            block_sum2<ASYNC>(sw, sww, red2, buf2);
             const double mean = sw / (double)V;
             const double bb = fmax(fma(-(double)V * mean, mean, sww), 0.0);
             const double b = sqrt(bb);
@@ -280,44 +390,46 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) lanczos_kernel(cons
             ++k;
             const bool breakdown = b < 1e-13 * (4.0 * DIM);
             if (breakdown || k == kmax || k == next_check) {
-                __syncthreads();
-                if (tid < 32) {
-                    // Ritz values decrease with k (interlacing): the new one lies below the last; a lower end a few
-                    // times the last decrease below it is tried first (one Sturm count says whether it holds)
-                    double lo_try = -(4.0 * DIM + 1.0);
-                    if (have_drop) {
-                        const double cand = lam - 8.0 * last_drop - 1e-9;
-                        if (sturm_count(alpha, beta2, k, cand) == 0) lo_try = cand;
+                const bool final = breakdown || k == kmax;
+                if (ASYNC) {
+                    int vk, vstep;
+                    double vlam, vres;
+                    rendezvous(k, (n_handed == 0 ? 1 : 0) | (final ? 2 : 0) | (breakdown ? 4 : 0), vk, vstep, vlam, vres);
+                    if (n_handed > 0 && vres < 1e-10) {   // the previous test passed: the steps since are discarded
+                        lam = vlam;
+                        k_out = vk;
+                        done = true;
+                    } else if (final) {                   // wait for this last test
+                        rendezvous(0, 0, vk, vstep, vlam, vres);
+                        lam = vlam;
+                        k_out = k;
+                        unconverged = !breakdown && !(vres < 1e-10) && k < V - 1;   // k = V-1: the Krylov space is the whole of 1-perp, T_k is exact
+                        done = true;
+                    } else {
+                        const int pred = n_handed > 0 ? vk + vstep : k + max(4, k / 4);
+                        next_check = max(k + 3, pred);
                     }
-                    // the Ritz value to 1e-11 is enough to follow the residual; it is refined to 2e-14 once the test passes
-                    double l = smallest_ritz(alpha, beta2, k, lo_try, lam_hi, 1e-11);
-                    const double res = breakdown ? 0.0 : b * last_component(alpha, beta, ibeta, k, l - 1e-13);
-                    if (breakdown || k == kmax || res < 1e-10) l = smallest_ritz(alpha, beta2, k, l - 2e-11 * fmax(1.0, fabs(l)), l + 2e-11 * fmax(1.0, fabs(l)), 2e-14);
-                    if (tid == 0) {
-                        s_lam = l;
-                        s_res = res;
+                    ++n_handed;
+                } else {
+                    __syncthreads();
+                    if (tid < 32) {
+                        double l, res;
+                        int step;
+                        ritz_test<DIM>(R, alpha, beta, beta2, ibeta, k, breakdown, final, l, res, step);
+                        if (tid == 0) {
+                            mail.v_lam = l;
+                            mail.v_res = res;
+                            mail.v_step = step;
+                        }
                     }
+                    __syncthreads();
+                    lam = mail.v_lam;
+                    const double res = mail.v_res;
+                    k_out = k;
+                    if (final || res < 1e-10) done = true;
+                    unconverged = !breakdown && !(res < 1e-10) && k < V - 1;   // k = V-1: the Krylov space is the whole of 1-perp, T_k is exact
+                    next_check = k + mail.v_step;
                 }
-                __syncthreads();
-                if (n_checks > 0) {
-                    last_drop = fmax(lam - s_lam, 0.0);
-                    have_drop = true;
-                }
-                lam = s_lam;
-                lam_hi = lam + 1e-9;
-                const double res = s_res;
-                if (breakdown || k == kmax || res < 1e-10) done = true;
-                unconverged = !breakdown && !(res < 1e-10) && k < V - 1;   // k = V-1: the Krylov space is the whole of 1-perp, T_k is exact
-                // next test where the residual bound, which falls geometrically, is expected to cross 1e-10
-                int step = max(4, k / 4);
-                if (n_checks > 0 && res > 0.0 && res < res_prev) {   // (a measured decay may carry the next test up to k/2 ahead)
-                    const double per_step = log(res_prev / res) / (double)(k - k_prev);
-                    step = max(3, min(max(4, k / 2), (int)(0.9 * log(res / 1e-10) / per_step) + 1));
-                }
-                res_prev = res;
-                k_prev = k;
-                ++n_checks;
-                next_check = k + step;
             }
             if (!done) {
                 const double ib = 1.0 / b;
@@ -330,7 +442,7 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) lanczos_kernel(cons
                 v0 = v1;
                 v1 = tmp;
                 beta_prev = b;
-                __syncthreads();
+                compute_barrier<ASYNC>();
             }
         }
         if (tid == 0) {
@@ -339,9 +451,14 @@ __global__ void __launch_bounds__(MAXT, MAXT <= 256 ? 2 : 1) lanczos_kernel(cons
             // bit 2: the step cap was reached with the residual bound still above 1e-10 (R16): lambda1 is then only an
             // upper bound of the eigenvalue and the caller should not trust a region of 1 or 2
             P.region[cfg] = (uint8_t)(reg | (unconverged ? 4 : 0));
-            if (P.steps) P.steps[cfg] = k;
+            if (P.steps) P.steps[cfg] = k_out;
             if (reg) atomicAdd(P.n_in, 1ull);
         }
+    }
+    if (ASYNC) {   // release the Ritz warp
+        int vk, vstep;
+        double vlam, vres;
+        rendezvous(-1, 0, vk, vstep, vlam, vres);
     }
 }
 
@@ -364,16 +481,28 @@ int launch(const u1gf_orbit* o, const FpParams& P, cudaStream_t st) {
     const int spt = V <= 128 ? 2 : (V <= U1GF_FP_SPT4_MAXV ? 4 : 8);
     const int T = ((V + spt - 1) / spt + 31) / 32 * 32;
     // the thread count bounds the registers ptxas may use
-    auto kern = spt == 8 ? (T <= 256 ? lanczos_kernel<DIM, 8, 256> : lanczos_kernel<DIM, 8, 640>)
-                         : (spt == 4 ? (T <= 256 ? lanczos_kernel<DIM, 4, 256> : lanczos_kernel<DIM, 4, 640>) : lanczos_kernel<DIM, 2, 256>);
+    // the large lattices (8 sites per thread: one or two CTAs per SM) run the Ritz test on a warp of its own
+#ifndef U1GF_FP_NO_ASYNC
+    const bool async = spt == 8;
+#else
+    const bool async = false;
+#endif
+    auto kern = spt == 8 ? (async ? (T <= 192 ? lanczos_kernel<DIM, 8, 192, true>      // 6^4: 144 registers at two CTAs per SM
+                                     : T <= 256 ? lanczos_kernel<DIM, 8, 256, true>
+                                     : T <= 512 ? lanczos_kernel<DIM, 8, 512, true>    // 8^4
+                                                : lanczos_kernel<DIM, 8, 640, true>)
+                                  : (T <= 256 ? lanczos_kernel<DIM, 8, 256, false> : lanczos_kernel<DIM, 8, 640, false>))
+                         : (spt == 4 ? (T <= 256 ? lanczos_kernel<DIM, 4, 256, false> : lanczos_kernel<DIM, 4, 640, false>)
+                                     : lanczos_kernel<DIM, 2, 256, false>);
+    const int threads = T + (async ? 32 : 0);
     if (T > 640) return fail(U1GF_EINVAL, "u1gf_check_fp: lattice of %d sites does not fit the resident Lanczos kernel", V);
     if (smem > 48 * 1024) U1GF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
-    U1GF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T, smem));
+    U1GF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
     if (per_sm < 1) return fail(U1GF_ECUDA, "u1gf_check_fp: kernel does not fit on an SM");
     unsigned long long grid = (unsigned long long)per_sm * o->sm_count;
     if (grid > P.n_cfg) grid = P.n_cfg;
-    kern<<<(unsigned)grid, T, smem, st>>>(o->dev, P);
+    kern<<<(unsigned)grid, threads, smem, st>>>(o->dev, P);
     U1GF_CUDA(cudaGetLastError());
     ++t_launches;
     return U1GF_OK;
