@@ -88,7 +88,7 @@ struct TG {
     static constexpr size_t off_lnk = off_x3 + (size_t)ST * 2 * SHEET_B;
     static constexpr size_t off_bar = off_lnk + (size_t)ST * LNK_B;           // fullW[RW], fullS[ST], empty[ST]
     static constexpr size_t off_sred = off_bar + (size_t)(RW + 2 * ST) * 8 + 8;
-    static constexpr size_t off_red = off_sred + (size_t)3 * CW * 32 * 8;   // [2][CW][32] sweep sums, [CW][32] odd sums
+    static constexpr size_t off_red = off_sred + (size_t)(5 * CW + 1) * 32 * 8;   // [2][CW][32] sweep sums, [CW][32] odd sums, [2][CW][32] F sums, [32] F of the lanes that stop
     static constexpr size_t off_pos = off_red + (size_t)2 * (CW + 1) * 5 * 8;
     static constexpr size_t off_skip = off_pos + 32 * 8;
     static constexpr size_t smem_bytes = off_skip + 32 * 4 + 16;
@@ -215,7 +215,7 @@ struct Smem {
 template <int N, int PAR, bool W1>
 __device__ __forceinline__ double half_sweep(const Smem<N>& S, const double2* src, double2* dst, double2* save,
                                              const double2* __restrict__ oth, const double2* __restrict__ lnk, unsigned hs,
-                                             int warp, int lane, double k2, bool commit, bool cand, bool& skipped) {
+                                             int warp, int lane, double k2, bool commit, bool cand, bool& skipped, double& accF) {
     using G = TG<N>;
     constexpr int H = G::H, SITES = G::SITES, SPW = G::SPW, CW = G::CW, NS = G::NS, WL = G::WL, RW = G::RW, ST = G::ST;
     const unsigned step0 = hs * NS, wl0 = hs * WL;
@@ -386,6 +386,11 @@ __device__ __forceinline__ double half_sweep(const Smem<N>& S, const double2* sr
             if (PAR == 0) {
                 const double dl = fma(gi.y, wr, -gi.x * wi);   // Delta_i of the field after sweep t
                 acc = fma(dl, dl, acc);
+                // a5: every link joins an even and an odd site, so the sum over the even sites of Re(g_i conj w_i) on the
+                // field before this update is F = sum_{i,mu} Re(g_i U_{i,mu} conj g_{i+mu}) of the field after sweep t
+                // (Eq. 3): two FMAs per even site instead of four gathered neighbours in the finalisation
+                accF = fma(gi.x, wr, accF);
+                accF = fma(gi.y, wi, accF);
             }
             bool sk;
             const double2 gn = site_update<W1>(gi, wr, wi, k2, sk);
@@ -421,6 +426,8 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* sred = reinterpret_cast<double*>(smem_raw + G::off_sred);              // [2][CW][32]
     double* sredO = sred + 2 * CW * 32;                                            // [CW][32]
+    double* sredF = sredO + CW * 32;                                               // [2][CW][32]
+    double* s_F = sredF + 2 * CW * 32;                                             // [32]
     double* red = reinterpret_cast<double*>(smem_raw + G::off_red);                // [2][NW][5]
     unsigned long long* s_pos = reinterpret_cast<unsigned long long*>(smem_raw + G::off_pos);
     unsigned* s_skip = reinterpret_cast<unsigned*>(smem_raw + G::off_skip);
@@ -478,20 +485,13 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
                 locate<N>(V - 1, pc, rc);
                 const double2 c = (pc ? O : SV)[(size_t)rc * 32 + L];
                 double v[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+#ifdef U1GF_TMA_PROF
+                const long long prof_f0 = clock64();
+#endif
                 for (int i = tid; i < V; i += THREADS) {
                     int pi, ri;
                     locate<N>(i, pi, ri);
                     const double2 gi = (pi ? O : SV)[(size_t)ri * 32 + L];
-                    const double2* Nb = pi ? SV : O;   // neighbours have the other parity
-#pragma unroll
-                    for (int mu = 0; mu < 4; ++mu) {   // F = sum Re(g_i U_{i,mu} conj g_{i+mu})   (Eq. 3)
-                        const double2 u = __ldg(D.U + i * 4 + mu);
-                        int pj, rj;
-                        locate<N>(__ldg(D.fwd + i * 4 + mu), pj, rj);
-                        const double2 gj = Nb[(size_t)rj * 32 + L];
-                        const double ar = fma(gi.x, u.x, -gi.y * u.y), ai = fma(gi.x, u.y, gi.y * u.x);
-                        v[0] += fma(ar, gj.x, ai * gj.y);
-                    }
                     const double re = fma(gi.x, c.x, gi.y * c.y);   // g~ = g conj(g_{V-1})
                     const double im = fma(gi.y, c.x, -gi.x * c.y);
                     const unsigned bits = __ldg(D.sgn + i);
@@ -501,9 +501,12 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
                     v[4] += ((bits & 8u) ? re : -re) + ((bits & 128u) ? im : -im);
                     if (P.g_canon) reinterpret_cast<double2*>(P.g_canon)[k * (unsigned long long)V + i] = make_double2(re, im);
                 }
+#ifdef U1GF_TMA_PROF
+                if (blockIdx.x == 0 && tid == 0) atomicAdd(&g_prof[4], (unsigned long long)(clock64() - prof_f0));
+#endif
                 block_sum<5, NW>(v, red, fb);   // its barrier also publishes the s_skip bits
                 if (tid == 0) {
-                    P.F_norm[k] = v[0] / (4.0 * (double)V);
+                    P.F_norm[k] = s_F[L] / (4.0 * (double)V);   // a5 came out of the last even half-sweep
                     P.sweeps[k] = tL;
                     P.status[k] = (uint8_t)((mxL ? 1 : 0) | (s_skip[L] ? 2 : 0));
                     reinterpret_cast<double4*>(P.sig)[k] =
@@ -516,6 +519,9 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
             const unsigned long long k = s_k;
             if (k < P.n_starts) {
                 const uint64_t s = P.start_ids ? P.start_ids[k] : P.first_start + k;
+#ifdef U1GF_TMA_PROF
+                const long long prof_r0 = clock64();
+#endif
                 for (int i = tid; i < V; i += THREADS) {   // a2: Philox counter (site, start lo, start hi, 0)
                     const u32x4 r = philox((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 0u, (uint32_t)P.seed,
                                            (uint32_t)(P.seed >> 32));
@@ -525,6 +531,9 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
                     locate<N>(i, pi, ri);
                     (pi ? O : E)[(size_t)ri * 32 + L] = make_double2(cs, sn);
                 }
+#ifdef U1GF_TMA_PROF
+                if (blockIdx.x == 0 && tid == 0) atomicAdd(&g_prof[5], (unsigned long long)(clock64() - prof_r0));
+#endif
                 if (tid == 0) {
                     s_pos[L] = k;
                     s_skip[L] = 0u;
@@ -551,7 +560,8 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
             fence_proxy_async();
             __syncthreads();
             PROF_T0();
-            accO = half_sweep<N, 1, W1>(S, O, O, nullptr, E, P.lnk + (size_t)HALF * 8, hs, warp, lane, P.k2, commit, false, skipped);
+            double unusedF = 0.0;
+            accO = half_sweep<N, 1, W1>(S, O, O, nullptr, E, P.lnk + (size_t)HALF * 8, hs, warp, lane, P.k2, commit, false, skipped, unusedF);
             if (warp == 0) { PROF_ADD(2); }
             hs = (hs + 1) % G::HSMOD;   // the mbarrier phases only need hs modulo a multiple of 2 RW and 2 ST
             if (commit) ++t;
@@ -566,25 +576,33 @@ __global__ void __launch_bounds__(TG<N>::THREADS, 1) relax_tma_kernel(const TmaP
 #pragma unroll
         for (int w = 0; w < CW; ++w) sumO += sredO[w * 32 + lane];
         const bool cand = active && t > 0 && ((t % P.check_every == 0 && sumO / (double)V < P.eps) || t == P.max_sweeps);
-        const double accE = half_sweep<N, 0, W1>(S, E, E, SV, O, P.lnk, hs, warp, lane, P.k2, active, cand, skipped);
+        double accF = 0.0;
+        const double accE = half_sweep<N, 0, W1>(S, E, E, SV, O, P.lnk, hs, warp, lane, P.k2, active, cand, skipped, accF);
         hs = (hs + 1) % G::HSMOD;
-        // a4: gauge precision of the field after sweep t (R5), fixed summation order over the warps
-        if (warp < CW) sred[(rb * CW + warp) * 32 + lane] = accE;
+        // a4: gauge precision of the field after sweep t (R5), a5: F of that field; fixed summation order over the warps
+        if (warp < CW) {
+            sred[(rb * CW + warp) * 32 + lane] = accE;
+            sredF[(rb * CW + warp) * 32 + lane] = accF;
+        }
         __syncthreads();
-        double Ssum = sumO;
+        double Ssum = sumO, Fsum = 0.0;
 #pragma unroll
-        for (int w = 0; w < CW; ++w) Ssum += sred[(rb * CW + w) * 32 + lane];
+        for (int w = 0; w < CW; ++w) {
+            Ssum += sred[(rb * CW + w) * 32 + lane];
+            Fsum += sredF[(rb * CW + w) * 32 + lane];
+        }
         rb ^= 1;
         const bool conv = active && t > 0 && (t % P.check_every == 0) && (Ssum / (double)V < P.eps);
         maxed = active && !conv && t == P.max_sweeps;
         dumpm = __ballot_sync(FULL, conv || maxed);
         need = dumpm;
+        if (warp == 0 && (conv || maxed)) s_F[lane] = Fsum;   // read by thread 0 behind the barriers of the finalisation
     }
 #ifdef U1GF_TMA_PROF
     __syncthreads();
     if (blockIdx.x == 0 && tid == 0)
-        printf("prof N=%d: producer waits on empty %llu, warp 0 waits on full %llu, odd half-sweeps (warp 0) %llu, service %llu cycles\n", N,
-               g_prof[0], g_prof[1], g_prof[2], g_prof[3]);
+        printf("prof N=%d: producer waits on empty %llu, warp 0 waits on full %llu, odd half-sweeps (warp 0) %llu, service %llu cycles "
+               "(finalisation loop of thread 0 %llu, refill loop %llu)\n", N, g_prof[0], g_prof[1], g_prof[2], g_prof[3], g_prof[4], g_prof[5]);
 #endif
 }
 
