@@ -179,6 +179,43 @@ int u1gf_paper_count(uint64_t n, const double* F_norm, const uint8_t* status, do
                      void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------------------
+ * u1gf_paper_count_static: u1gf_paper_count for callers that have no way to obtain device memory.
+ *
+ * Every other device-pointer call of this header wants a workspace from the caller, and the *_host calls allocate
+ * one inside.  Neither works for code that was handed its input and output buffers by a host application and nothing
+ * else: a plug-in inside a simulation whose driver carved up the whole of HBM at start-up and forbids (or would
+ * fail) a later cudaMalloc; a measurement step inside a latency-critical loop, where cudaMalloc / cudaFree would
+ * stall every stream of the device while they run; an embedding that may issue stream work only and has no
+ * allocator of its own to ask.  For those, the scratch of this one call is built into the library: a fixed
+ * 32 MiB array in device memory (`static __device__`, 256-byte aligned) that belongs to the library's device code.
+ * Each GPU onto which that code is loaded holds those 32 MiB until the process exits, whether the call is ever made
+ * or not.
+ *
+ *   n        number of records, 0 <= n <= U1GF_PAPER_COUNT_STATIC_MAX_N (2^20, one "mebisample" of PAPER.md:L131);
+ *            a larger n is refused with U1GF_EINVAL and a message naming the limit -- use u1gf_paper_count then
+ *   F_norm   dev [n], status dev [n], scale, n_keys dev [1] int64: exactly as u1gf_paper_count; the result is the same
+ *            integer (same kernels, same sort, only the scratch differs).  Inputs and output stay the caller's.
+ *   Set-up   the FIRST call on each device looks up where the array lives on that device (cudaGetSymbolAddress,
+ *            return code checked, address kept per device ordinal).  That look-up can make the runtime load this
+ *            library's device code onto the GPU, so make the first call on a device early -- with that device
+ *            current, and before any stream capture is begun; n = 0 is enough (it does the set-up, zeroes n_keys and
+ *            launches nothing else).  Later calls only enqueue a memset, two kernels and the radix sort on the stream.
+ *   Allocation  none: no cudaMalloc, cudaFree or allocating library routine anywhere on this path, first call included
+ *            (the sort gets its temporary storage from the array).
+ *   Sharing  there is ONE array per GPU and every call uses it.  Calls on the same stream are ordered and safe.  Two
+ *            calls that can overlap on the GPU (different streams without an event between them, or several host
+ *            threads on different streams) race on it and return garbage counts -- serialise them.  The array keeps
+ *            whatever the previous call left; the call relies on none of it (both key arrays are rewritten for all n
+ *            records and the sort clears its own counters), and n_keys is zeroed on the stream first.
+ * Errors: U1GF_EINVAL (NULL pointer, scale <= 0, n over the limit, device ordinal >= 64), U1GF_ENODEV, U1GF_ECUDA;
+ *         U1GF_ENOMEM only if the sort asked for more temporary storage than the array leaves (not on sm_100a).
+ * Asynchronous on the stream like the other device-pointer calls.
+ * ------------------------------------------------------------------------------------------------------- */
+#define U1GF_PAPER_COUNT_STATIC_MAX_N 1048576
+int u1gf_paper_count_static(uint64_t n, const double* F_norm, const uint8_t* status, double scale, int64_t* n_keys,
+                            void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------------------
  * The whole hot path in one call with HOST result buffers (what an application that keeps nothing on the device
  * calls, and what bench.py's `e2e` times): u1gf_relax_batch on all starts -> u1gf_count_copies -> the representatives
  * re-relaxed with their fields -> u1gf_check_fp.  Intermediates never leave the device; device scratch comes from a

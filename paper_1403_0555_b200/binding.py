@@ -39,6 +39,7 @@ _SIGNATURES = {
     "u1gf_discovery_curve": (C.c_int, [C.c_uint64, _p, C.c_int32, _p, _p]),
     "u1gf_paper_count_workspace_bytes": (C.c_size_t, [C.c_uint64]),
     "u1gf_paper_count": (C.c_int, [C.c_uint64, _p, _p, C.c_double, _p, _p, C.c_size_t, _p]),
+    "u1gf_paper_count_static": (C.c_int, [C.c_uint64, _p, _p, C.c_double, _p, _p]),
     "u1gf_pipeline_host": (C.c_int, [_p, C.c_uint64, C.c_uint64, C.c_uint64, C.c_double, C.c_double, C.c_int32, C.c_int32,
                                      C.c_double, C.c_double, C.c_double, C.c_int32, _p, _p, _p, _p, _p, C.c_int64, _p, _p,
                                      _p, _p, _p, _p, _p, _p]),
@@ -457,6 +458,23 @@ def paper_count(F_norm, status, scale=1e8, workspace=None):
     _check(lib().u1gf_paper_count(n, _dev_ptr(F_norm), _dev_ptr(status), float(scale), _dev_ptr(nk),
                                   _aligned_ptr(workspace), need, _stream()))
     return nk
+
+
+PAPER_COUNT_STATIC_MAX_N = 1 << 20   # U1GF_PAPER_COUNT_STATIC_MAX_N of include/u1gf.h
+
+
+def paper_count_static(F_norm, status, scale=1e8, out=None):
+    """u1gf_paper_count_static: the count of u1gf_paper_count for callers that cannot get device memory (all of it handed
+    out by their host application, no allocator to ask, or an allocation stall they cannot afford): the scratch is a
+    32 MiB array built into the library, so nothing is allocated here either when `out` (device int64 [1]) is given.
+    At most PAPER_COUNT_STATIC_MAX_N records; every call shares the one array, so calls must not overlap on the GPU.
+    The first call on a device does the set-up (include/u1gf.h) -- make it before any stream capture."""
+    n = int(F_norm.numel())
+    if out is None:
+        import torch
+        out = torch.empty(1, dtype=torch.int64, device="cuda")
+    _check(lib().u1gf_paper_count_static(n, _dev_ptr(F_norm), _dev_ptr(status), float(scale), _dev_ptr(out), _stream()))
+    return out
 
 
 def _mcheck(rc):

@@ -10,6 +10,8 @@
 // Integer work only; no floating-point atomics.
 #include <cub/device/device_radix_sort.cuh>
 
+#include <mutex>
+
 #include "u1gf_internal.h"
 
 namespace u1gf {
@@ -68,6 +70,51 @@ size_t sort_temp_bytes(uint64_t n) {
 }  // namespace
 }  // namespace u1gf
 
+// ---------------------------------------------------------------------------------------------------------------------
+// Scratch for u1gf_paper_count_static (see include/u1gf.h).  The array is part of this library's device image: each GPU
+// on which this file's device code gets loaded keeps kStaticScratchBytes of it until the process exits, used or not.
+// Layout during a call: keys [n] | sorted keys [n] | CUB sort temporary -- the layout u1gf_paper_count puts in the
+// caller's workspace.  Nothing in it has to be zero when a call starts: both key arrays are overwritten in full for
+// i < n before they are read, and the sort zeroes the counters it keeps in its temporary itself.  The only value that
+// must start at zero is the caller's n_keys, which the entry point clears on the stream.
+//
+// `g_static_scratch` written in HOST code is the host-side shadow of the symbol, not where the array lives on the GPU;
+// static_scratch_address() asks the runtime for the real address once per device and keeps it.
+// ---------------------------------------------------------------------------------------------------------------------
+static constexpr size_t kStaticMaxN = (size_t)U1GF_PAPER_COUNT_STATIC_MAX_N;
+// 2 key arrays of kStaticMaxN 8-byte keys (16 MiB) + the sort's temporary, a third key array plus its digit counters
+// (tests/test_zz_no_alloc.py runs the full kStaticMaxN on the GPU, so a sort that wanted more would be caught).  32 MiB.
+static constexpr size_t kStaticScratchBytes = 4 * kStaticMaxN * sizeof(unsigned long long);
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+namespace u1gf {
+namespace {
+
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mutex;
+void* g_static_address[kMaxDevices] = {};   // device address of g_static_scratch on device k, NULL = not looked up yet
+
+// Device address of the array on the CURRENT device.  The first call per device is the set-up: cudaGetSymbolAddress may
+// have to load this file's device code onto that GPU, which is when the array comes into existence there.
+int static_scratch_address(void** out) {
+    int dev = -1;
+    U1GF_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices)
+        return fail(U1GF_EINVAL, "u1gf_paper_count_static: device ordinal %d outside 0..%d", dev, kMaxDevices - 1);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_address[dev]) {
+        void* p = nullptr;
+        U1GF_CUDA(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p) return fail(U1GF_ECUDA, "u1gf_paper_count_static: cudaGetSymbolAddress returned a NULL address on device %d", dev);
+        g_static_address[dev] = p;
+    }
+    *out = g_static_address[dev];
+    return U1GF_OK;
+}
+
+}  // namespace
+}  // namespace u1gf
+
 using namespace u1gf;
 
 extern "C" {
@@ -115,6 +162,44 @@ int u1gf_paper_count(uint64_t n, const double* F_norm, const uint8_t* status, do
     count_runs_kernel<<<blocks, 256, 0, st>>>((unsigned long long)n, k1, (unsigned long long*)n_keys);
     U1GF_CUDA(cudaGetLastError());
     t_launches += 2;   // own kernels; the CUB sort launches are library code and not counted
+    return U1GF_OK;
+}
+
+// The same three steps as u1gf_paper_count (keys -> radix sort -> count run heads), with the scratch taken from
+// g_static_scratch instead of a caller workspace.  No cudaMalloc / cudaFree / allocating library call on this path:
+// cudaMemsetAsync, kernel launches and cub::DeviceRadixSort::SortKeys with its temporary storage handed in.
+int u1gf_paper_count_static(uint64_t n, const double* F_norm, const uint8_t* status, double scale, int64_t* n_keys,
+                            void* cuda_stream) {
+    t_launches = 0;
+    if (!n_keys) return fail(U1GF_EINVAL, "u1gf_paper_count_static: NULL n_keys");
+    if (!(scale > 0.0)) return fail(U1GF_EINVAL, "u1gf_paper_count_static: scale must be > 0");
+    if (n > (uint64_t)kStaticMaxN)
+        return fail(U1GF_EINVAL,
+                    "u1gf_paper_count_static: n = %llu exceeds U1GF_PAPER_COUNT_STATIC_MAX_N = %llu, the size the built-in "
+                    "scratch array was compiled for; use u1gf_paper_count with a caller workspace for larger batches",
+                    (unsigned long long)n, (unsigned long long)kStaticMaxN);
+    if (n && (!F_norm || !status)) return fail(U1GF_EINVAL, "u1gf_paper_count_static: NULL input array");
+    if (int rc = check_device()) return rc;
+    void* scratch = nullptr;
+    if (int rc = static_scratch_address(&scratch)) return rc;   // first call on this device: the set-up
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    U1GF_CUDA(cudaMemsetAsync(n_keys, 0, sizeof(int64_t), st));
+    if (n == 0) return U1GF_OK;
+    const size_t kb = (((size_t)n * 8) + 255) & ~(size_t)255;
+    size_t tb = sort_temp_bytes(n);
+    if (2 * kb + tb > kStaticScratchBytes)
+        return fail(U1GF_ENOMEM, "u1gf_paper_count_static: n = %llu needs %zu bytes of scratch, the built-in array holds %zu",
+                    (unsigned long long)n, 2 * kb + tb, kStaticScratchBytes);
+    unsigned long long* k0 = (unsigned long long*)scratch;
+    unsigned long long* k1 = (unsigned long long*)((char*)scratch + kb);
+    void* temp = (char*)scratch + 2 * kb;
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    paper_keys_kernel<<<blocks, 256, 0, st>>>((unsigned long long)n, F_norm, status, scale, k0);
+    U1GF_CUDA(cudaGetLastError());
+    U1GF_CUDA(cub::DeviceRadixSort::SortKeys(temp, tb, k0, k1, (unsigned long long)n, 0, 64, st));
+    count_runs_kernel<<<blocks, 256, 0, st>>>((unsigned long long)n, k1, (unsigned long long*)n_keys);
+    U1GF_CUDA(cudaGetLastError());
+    t_launches += 2;
     return U1GF_OK;
 }
 
