@@ -16,20 +16,33 @@ namespace {
 struct Arena {
     char* base = nullptr;
     size_t cap = 0, used = 0;
+    int device = -1;   // the device `base` was allocated on: a thread that switches device gets a fresh allocation there
     ~Arena() {
+        // at thread exit; at process exit the runtime may already be gone, then cudaFree reports an error we drop
         if (base) cudaFree(base);
+    }
+    void release() {
+        if (base) cudaFree(base);   // a device pointer identifies its own device: no cudaSetDevice needed
+        base = nullptr;
+        cap = used = 0;
+        device = -1;
     }
     bool reserve(size_t bytes) {
         used = 0;
-        if (bytes <= cap) return true;
-        if (base) cudaFree(base);
-        base = nullptr;
-        cap = 0;
-        if (cudaMalloc((void**)&base, bytes) != cudaSuccess) {
+        int dev = -1;
+        if (cudaGetDevice(&dev) != cudaSuccess) {
             cudaGetLastError();
             return false;
         }
+        if (base && dev == device && bytes <= cap) return true;
+        release();
+        if (cudaMalloc((void**)&base, bytes) != cudaSuccess) {
+            cudaGetLastError();
+            base = nullptr;
+            return false;
+        }
         cap = bytes;
+        device = dev;
         return true;
     }
     void* take(size_t bytes) {
@@ -40,6 +53,24 @@ struct Arena {
     static size_t padded(size_t bytes) { return (bytes + 255) & ~(size_t)255; }
 };
 thread_local Arena t_arena;
+
+// The tables of an orbit live on the device that was current in u1gf_create_orbit; the *_host calls allocate and launch
+// on the current device, so the two must agree.
+int same_device(const u1gf_orbit* o, const char* who) {
+    int dev = -1;
+    U1GF_CUDA(cudaGetDevice(&dev));
+    if (dev != o->device)
+        return fail(U1GF_EINVAL, "%s: the orbit was created on device %d, the current device is %d", who, o->device, dev);
+    return U1GF_OK;
+}
+
+// Error returns of u1gf_pipeline_host must not leave copies into the caller's host arrays in flight.
+struct DrainUnlessDone {
+    bool done = false;
+    ~DrainUnlessDone() {
+        if (!done) cudaDeviceSynchronize();
+    }
+};
 
 struct DevBuf {   // a slice of the arena
     void* p = nullptr;
@@ -63,9 +94,7 @@ __global__ void gather_F_kernel(unsigned long long n, const int64_t* __restrict_
 extern "C" {
 
 int u1gf_release_host_scratch(void) {
-    if (t_arena.base) cudaFree(t_arena.base);
-    t_arena.base = nullptr;
-    t_arena.cap = t_arena.used = 0;
+    t_arena.release();
     return U1GF_OK;
 }
 
@@ -75,6 +104,7 @@ int u1gf_relax_batch_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_sta
                           double* sig_host, double* g_canon_host) {
     if (!o) return fail(U1GF_EINVAL, "u1gf_relax_batch_host: NULL orbit");
     if (int rc = check_device()) return rc;
+    if (int rc = same_device(o, "u1gf_relax_batch_host")) return rc;
     if (n_starts == 0) return U1GF_OK;
     const size_t n = (size_t)n_starts, V = (size_t)o->dev.V;
     DevBuf F, sw, stt, sg, gc, ids, ws;
@@ -104,6 +134,7 @@ int u1gf_check_fp_host(const u1gf_orbit* o, uint64_t n_cfg, const double* g_host
                        double* lambda1_host, uint8_t* region_host, int64_t* n_in_region_host) {
     if (!o || !g_host) return fail(U1GF_EINVAL, "u1gf_check_fp_host: NULL argument");
     if (int rc = check_device()) return rc;
+    if (int rc = same_device(o, "u1gf_check_fp_host")) return rc;
     const size_t n = (size_t)n_cfg, V = (size_t)o->dev.V;
     DevBuf g, lam, reg, cnt;
     if (!t_arena.reserve(Arena::padded(n * V * 16) + Arena::padded(n * 8) + Arena::padded(n) + 1024))
@@ -168,6 +199,7 @@ int u1gf_pipeline_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_start,
     if (copy_capacity < 0 || nbins < 0) return fail(U1GF_EINVAL, "u1gf_pipeline_host: negative capacity");
     if (n_starts >= (1ull << 31)) return fail(U1GF_EINVAL, "u1gf_pipeline_host: n_starts must be below 2^31");
     if (int rc = check_device()) return rc;
+    if (int rc = same_device(o, "u1gf_pipeline_host")) return rc;
     *n_distinct_host = 0;
     *n_in_region_host = 0;
     if (n_starts == 0) return U1GF_OK;
@@ -193,6 +225,7 @@ int u1gf_pipeline_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_start,
     int64_t* nd_dev = (int64_t*)cnt.p;
     int64_t* nin_dev = nd_dev + 1;
     int launches = 0;
+    DrainUnlessDone drain;
     // a2-a6 on every start, a8
     int rc = u1gf_relax_batch(o, seed, first_start, n_starts, nullptr, omega, eps, max_sweeps, check_every, (double*)F.p,
                               (int32_t*)sw.p, (uint8_t*)stt.p, (double*)sg.p, nullptr, wsb.p, ws, nullptr);
@@ -206,6 +239,10 @@ int u1gf_pipeline_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_start,
     int64_t nd = 0;
     U1GF_CUDA(cudaMemcpy(&nd, nd_dev, 8, cudaMemcpyDeviceToHost));   // the one host read the path needs
     *n_distinct_host = nd;
+    const bool want_tables = rep_host || multiplicity_host || F_rep_host || lambda1_host || region_host;
+    if (want_tables && nd > copy_capacity)     // before any copy into the caller's arrays is enqueued
+        return fail(U1GF_ENOMEM, "u1gf_pipeline_host: %lld distinct copies, per-copy arrays hold %lld", (long long)nd,
+                    (long long)copy_capacity);
     // per-start results travel while the representatives are processed
     if (F_norm_host) U1GF_CUDA(cudaMemcpyAsync(F_norm_host, F.p, n * 8, cudaMemcpyDeviceToHost, nullptr));
     if (sweeps_host) U1GF_CUDA(cudaMemcpyAsync(sweeps_host, sw.p, n * 4, cudaMemcpyDeviceToHost, nullptr));
@@ -213,10 +250,6 @@ int u1gf_pipeline_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_start,
     if (sig_host) U1GF_CUDA(cudaMemcpyAsync(sig_host, sg.p, n * 32, cudaMemcpyDeviceToHost, nullptr));
     if (copy_id_host) U1GF_CUDA(cudaMemcpyAsync(copy_id_host, cid.p, n * 4, cudaMemcpyDeviceToHost, nullptr));
     if (hist_host && nbins > 0) U1GF_CUDA(cudaMemcpyAsync(hist_host, hist.p, hb, cudaMemcpyDeviceToHost, nullptr));
-    const bool want_tables = rep_host || multiplicity_host || F_rep_host || lambda1_host || region_host;
-    if (want_tables && nd > copy_capacity)
-        return fail(U1GF_ENOMEM, "u1gf_pipeline_host: %lld distinct copies, per-copy arrays hold %lld", (long long)nd,
-                    (long long)copy_capacity);
     // a7 on the representatives: re-relaxed with their fields written out (a start is a pure function of its index)
     int64_t n_in = 0;
     for (int64_t a = 0; a < nd; a += (int64_t)chunk) {
@@ -250,6 +283,7 @@ int u1gf_pipeline_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_start,
         if (region_host) U1GF_CUDA(cudaMemcpyAsync(region_host, reg.p, (size_t)nd, cudaMemcpyDeviceToHost, nullptr));
     }
     U1GF_CUDA(cudaDeviceSynchronize());
+    drain.done = true;
     t_launches = launches;
     return U1GF_OK;
 }
