@@ -119,7 +119,10 @@ const char* u1gf_kernel_name(const u1gf_orbit* o);
  *   tol_fp      region bits 0-1 = 1 if lambda_1 > tol_fp (inside), 2 if |lambda_1| <= tol_fp (marginal, "semi"definite),
  *               0 if lambda_1 < -tol_fp (outside); region bit 2 (value 4) is set when the iteration reached its cap of
  *               min(V-1, 512) steps with the Ritz residual bound still above 1e-10 (R16): lambda1 is then only an upper
- *               bound of the eigenvalue, and an "inside" verdict is not proven
+ *               bound of the eigenvalue, and an "inside" verdict is not proven.  Lattices with V-1 <= 512 never get bit 2: a run
+ *               that reaches k = V-1 has used up the whole space orthogonal to the constant mode and is taken as exact.
+ *               That holds in exact arithmetic only (the iteration does not reorthogonalise); on such lattices lambda1
+ *               has been within 1e-8 of the dense eigenvalue in every test, but the verdict is not proven by a bound
  *   lambda1     dev [n_cfg];  region dev [n_cfg];  n_in_region dev [1] = number of configurations with (region & 3) != 0
  *   lanczos_steps  dev [n_cfg] int32 or NULL: Lanczos steps taken per configuration
  * A converged relaxation can stop at a saddle it is still leaving (the stop rule tests the gradient only):
@@ -217,8 +220,13 @@ int u1gf_paper_count_static(uint64_t n, const double* F_norm, const uint8_t* sta
 
 /* ---------------------------------------------------------------------------------------------------------
  * The whole hot path in one call with HOST result buffers (what an application that keeps nothing on the device
- * calls, and what bench.py's `e2e` times): u1gf_relax_batch on all starts -> u1gf_count_copies -> the representatives
- * re-relaxed with their fields -> u1gf_check_fp.  Intermediates never leave the device; device scratch comes from a
+ * calls, and what bench.py's `e2e` times): u1gf_relax_batch on all starts -> u1gf_count_copies -> the fields of the
+ * representatives -> u1gf_check_fp.  Where those fields come from: normally the representatives are relaxed once more
+ * with g_canon written (in chunks of 1 GiB of fields).  The handle remembers whether its last call found
+ * n_distinct > n_starts/4 (a hot orbit: most starts are their own copy); if so, and n_starts*V*16 bytes are at most a
+ * quarter of the device memory, the next call writes the fields of ALL starts in the first pass and hands
+ * u1gf_check_fp cfg_index = rep, so nothing is relaxed twice.  Outputs are identical either way.
+ * Intermediates never leave the device; device scratch comes from a
  * grow-only per-thread allocation that is kept between calls (u1gf_release_host_scratch frees it; the other *_host
  * calls use the same scratch).
  *   per start (host [n_starts] or NULL): F_norm, sweeps, status, sig [n*4], copy_id
@@ -277,6 +285,11 @@ int u1gf_count_copies_ensemble(int32_t n_orbits, uint64_t n_per_orbit, const dou
  * the copy identity of u1gf_count_copies (R7).  Outputs: merged_id[e] = merged copy of entry e, merged copies numbered
  * by increasing first discovery; n_merged dev [1]; merged_first_start / merged_multiplicity dev [m], the first n_merged
  * entries valid.  The global copy id of a start is merged_id[offset of its range + its local copy id].
+ * Caveat: only the LEADERS of the ranges are clustered.  u1gf_count_copies on the undivided batch chains its F-runs
+ * through every member (adjacent gaps <= tol_F); two leaders of one copy whose F differ by more than tol_F, bridged
+ * there by other members, fall into different runs here and stay two merged copies.  The result equals the one-pass
+ * count whenever the F spread inside a copy is below tol_F -- at the default tol_F = 1e-10 against a spread of about
+ * 1e-13 after convergence to eps = 1e-13 that is the normal case; with a loose eps or a tight tol_F it is not guaranteed.
  * All arrays dev, int64 unless stated; workspace >= u1gf_merge_workspace_bytes(m), 256-byte aligned; asynchronous.
  * ------------------------------------------------------------------------------------------------------- */
 size_t u1gf_merge_workspace_bytes(uint64_t m);

@@ -1,8 +1,9 @@
 // host_calls.cu -- the *_host entry points of include/u1gf.h: host result buffers, device scratch from a per-thread
 // arena, copies inside the call, stream drained before returning.  u1gf_pipeline_host is the whole hot path in one call
-// (what bench.py's e2e leg times): relax -> count -> re-relax the representatives -> first-Gribov-region test, with
-// every intermediate staying on the device.
+// (what bench.py's e2e leg times): relax -> count -> fields of the representatives (relaxed once more on cold orbits, kept
+// from the first pass on hot ones) -> first-Gribov-region test, with every intermediate staying on the device.
 #include <algorithm>
+#include <vector>
 
 #include "u1gf_internal.h"
 
@@ -204,31 +205,49 @@ int u1gf_pipeline_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_start,
     *n_in_region_host = 0;
     if (n_starts == 0) return U1GF_OK;
     const size_t n = (size_t)n_starts, V = (size_t)o->dev.V;
-    // representatives are re-relaxed and tested in chunks whose fields fit a fixed budget
+    // Where do the fields of the representatives come from?  Cold orbits (few copies): the representatives are relaxed once
+    // more, with their fields written out, in chunks whose fields fit a fixed budget.  Hot orbits (most starts are their own
+    // copy; the previous call on this handle found n_distinct > n/4): the first pass writes the fields of ALL starts and
+    // u1gf_check_fp picks the representatives through cfg_index = rep -- nothing is relaxed twice.  The results are the same
+    // either way: a start is a pure function of its index.
     const size_t g_budget = (size_t)1 << 30;
     size_t chunk = std::max<size_t>(1, g_budget / (V * 16));
     if (chunk > n) chunk = n;
+    const size_t n_chunks = (n + chunk - 1) / chunk;
+    bool keep = false;
+    if (o->pipeline_keep_fields) {
+        size_t free_b = 0, total_b = 0;
+        U1GF_CUDA(cudaMemGetInfo(&free_b, &total_b));
+        keep = n * V * 16 <= total_b / 4;
+    }
     const size_t ws_relax = u1gf_relax_workspace_bytes(o, n_starts), ws_count = u1gf_count_workspace_bytes(n_starts);
     const size_t ws = std::max(ws_relax, ws_count);
     const size_t hb = (size_t)nbins * 8;
-    const size_t total = Arena::padded(n * 8) + Arena::padded(n * 4) + Arena::padded(n) + Arena::padded(n * 32) +
-                         Arena::padded(n * 4) + 3 * Arena::padded(n * 8) + Arena::padded(n * 8) + Arena::padded(n) +
-                         Arena::padded(hb) + Arena::padded(ws) + Arena::padded(chunk * V * 16) +
-                         Arena::padded(chunk * 8) + Arena::padded(chunk * 4) + 2 * Arena::padded(chunk) +
-                         Arena::padded(chunk * 32) + Arena::padded(chunk * 8) + 4096;
-    if (!t_arena.reserve(total)) return fail(U1GF_ENOMEM, "u1gf_pipeline_host: device allocation of %zu bytes failed", total);
+    const size_t cnt_bytes = (n_chunks + 2) * 8;
+    const size_t per_start = Arena::padded(n * 8) + Arena::padded(n * 4) + Arena::padded(n) + Arena::padded(n * 32) +
+                             Arena::padded(n * 4) + 3 * Arena::padded(n * 8) + Arena::padded(n * 8) + Arena::padded(n) +
+                             Arena::padded(hb) + Arena::padded(ws) + Arena::padded(cnt_bytes) + 4096;
+    const size_t redo = Arena::padded(chunk * V * 16) + Arena::padded(chunk * 8) + Arena::padded(chunk * 4) +
+                        2 * Arena::padded(chunk) + Arena::padded(chunk * 32) + Arena::padded(chunk * 8);
+    if (keep && !t_arena.reserve(per_start + Arena::padded(n * V * 16))) keep = false;   // does not fit beside the rest: chunks
+    if (!keep && !t_arena.reserve(per_start + redo))
+        return fail(U1GF_ENOMEM, "u1gf_pipeline_host: device allocation of %zu bytes failed", per_start + redo);
     DevBuf F, sw, stt, sg, cid, rep, mul, Frep, lam, reg, hist, wsb, gc, ids, sw2, st2, reg2, sg2, F2, cnt;
     F.take(n * 8); sw.take(n * 4); stt.take(n); sg.take(n * 32); cid.take(n * 4); rep.take(n * 8); mul.take(n * 8);
-    Frep.take(n * 8); lam.take(n * 8); reg.take(n); hist.take(hb); wsb.take(ws); gc.take(chunk * V * 16);
-    ids.take(chunk * 8); sw2.take(chunk * 4); st2.take(chunk); reg2.take(chunk); sg2.take(chunk * 32); F2.take(chunk * 8);
-    cnt.take(64);
+    Frep.take(n * 8); lam.take(n * 8); reg.take(n); hist.take(hb); wsb.take(ws); cnt.take(cnt_bytes);
+    if (keep) {
+        gc.take(n * V * 16);
+    } else {
+        gc.take(chunk * V * 16); ids.take(chunk * 8); sw2.take(chunk * 4); st2.take(chunk); reg2.take(chunk);
+        sg2.take(chunk * 32); F2.take(chunk * 8);
+    }
     int64_t* nd_dev = (int64_t*)cnt.p;
-    int64_t* nin_dev = nd_dev + 1;
+    int64_t* nin_dev = nd_dev + 1;     // one slot per u1gf_check_fp call, read back together at the end
     int launches = 0;
     DrainUnlessDone drain;
     // a2-a6 on every start, a8
     int rc = u1gf_relax_batch(o, seed, first_start, n_starts, nullptr, omega, eps, max_sweeps, check_every, (double*)F.p,
-                              (int32_t*)sw.p, (uint8_t*)stt.p, (double*)sg.p, nullptr, wsb.p, ws, nullptr);
+                              (int32_t*)sw.p, (uint8_t*)stt.p, (double*)sg.p, keep ? (double*)gc.p : nullptr, wsb.p, ws, nullptr);
     if (rc) return rc;
     launches += t_launches;
     rc = u1gf_count_copies(n_starts, (const double*)F.p, (const double*)sg.p, (const uint8_t*)stt.p, tol_F, tol_sig,
@@ -237,39 +256,51 @@ int u1gf_pipeline_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_start,
     if (rc) return rc;
     launches += t_launches;
     int64_t nd = 0;
-    U1GF_CUDA(cudaMemcpy(&nd, nd_dev, 8, cudaMemcpyDeviceToHost));   // the one host read the path needs
+    U1GF_CUDA(cudaMemcpy(&nd, nd_dev, 8, cudaMemcpyDeviceToHost));   // the one host read the path needs before it can go on
     *n_distinct_host = nd;
+    o->pipeline_keep_fields = (uint64_t)nd > n_starts / 4 ? 1 : 0;
     const bool want_tables = rep_host || multiplicity_host || F_rep_host || lambda1_host || region_host;
     if (want_tables && nd > copy_capacity)     // before any copy into the caller's arrays is enqueued
         return fail(U1GF_ENOMEM, "u1gf_pipeline_host: %lld distinct copies, per-copy arrays hold %lld", (long long)nd,
                     (long long)copy_capacity);
-    // per-start results travel while the representatives are processed
+    // per-start results: enqueued here, on the same (legacy default) stream as everything else, so they run before the
+    // first-region phase, not beside it; with pinned host arrays the host goes straight on to enqueue that phase
     if (F_norm_host) U1GF_CUDA(cudaMemcpyAsync(F_norm_host, F.p, n * 8, cudaMemcpyDeviceToHost, nullptr));
     if (sweeps_host) U1GF_CUDA(cudaMemcpyAsync(sweeps_host, sw.p, n * 4, cudaMemcpyDeviceToHost, nullptr));
     if (status_host) U1GF_CUDA(cudaMemcpyAsync(status_host, stt.p, n, cudaMemcpyDeviceToHost, nullptr));
     if (sig_host) U1GF_CUDA(cudaMemcpyAsync(sig_host, sg.p, n * 32, cudaMemcpyDeviceToHost, nullptr));
     if (copy_id_host) U1GF_CUDA(cudaMemcpyAsync(copy_id_host, cid.p, n * 4, cudaMemcpyDeviceToHost, nullptr));
     if (hist_host && nbins > 0) U1GF_CUDA(cudaMemcpyAsync(hist_host, hist.p, hb, cudaMemcpyDeviceToHost, nullptr));
-    // a7 on the representatives: re-relaxed with their fields written out (a start is a pure function of its index)
-    int64_t n_in = 0;
-    for (int64_t a = 0; a < nd; a += (int64_t)chunk) {
-        const uint64_t m = (uint64_t)std::min<int64_t>((int64_t)chunk, nd - a);
-        add_offset_kernel<<<(unsigned)((m + 255) / 256), 256>>>(m, (const int64_t*)rep.p + a, first_start, (uint64_t*)ids.p);
-        U1GF_CUDA(cudaGetLastError());
-        ++launches;
-        rc = u1gf_relax_batch(o, seed, 0, m, (const uint64_t*)ids.p, omega, eps, max_sweeps, check_every, (double*)F2.p,
-                              (int32_t*)sw2.p, (uint8_t*)st2.p, (double*)sg2.p, (double*)gc.p, wsb.p, ws, nullptr);
-        if (rc) return rc;
-        launches += t_launches;
-        rc = u1gf_check_fp(o, m, (const double*)gc.p, nullptr, tol_fp, (double*)lam.p + a, (uint8_t*)reg.p + a, nin_dev,
-                           nullptr, nullptr);
-        if (rc) return rc;
-        launches += t_launches;
-        int64_t part = 0;
-        U1GF_CUDA(cudaMemcpy(&part, nin_dev, 8, cudaMemcpyDeviceToHost));
-        n_in += part;
+    // a7 on the representatives
+    size_t fp_calls = 0;
+    if (keep) {
+        if (nd > 0) {
+            rc = u1gf_check_fp(o, (uint64_t)nd, (const double*)gc.p, (const int64_t*)rep.p, tol_fp, (double*)lam.p,
+                               (uint8_t*)reg.p, nin_dev, nullptr, nullptr);
+            if (rc) return rc;
+            launches += t_launches;
+            fp_calls = 1;
+        }
+    } else {
+        // re-relaxed with their fields written out (a start is a pure function of its index)
+        for (int64_t a = 0; a < nd; a += (int64_t)chunk) {
+            const uint64_t m = (uint64_t)std::min<int64_t>((int64_t)chunk, nd - a);
+            add_offset_kernel<<<(unsigned)((m + 255) / 256), 256>>>(m, (const int64_t*)rep.p + a, first_start, (uint64_t*)ids.p);
+            U1GF_CUDA(cudaGetLastError());
+            ++launches;
+            rc = u1gf_relax_batch(o, seed, 0, m, (const uint64_t*)ids.p, omega, eps, max_sweeps, check_every, (double*)F2.p,
+                                  (int32_t*)sw2.p, (uint8_t*)st2.p, (double*)sg2.p, (double*)gc.p, wsb.p, ws, nullptr);
+            if (rc) return rc;
+            launches += t_launches;
+            rc = u1gf_check_fp(o, m, (const double*)gc.p, nullptr, tol_fp, (double*)lam.p + a, (uint8_t*)reg.p + a,
+                               nin_dev + fp_calls, nullptr, nullptr);
+            if (rc) return rc;
+            launches += t_launches;
+            ++fp_calls;
+        }
     }
-    *n_in_region_host = n_in;
+    std::vector<int64_t> parts(fp_calls, 0);
+    if (fp_calls) U1GF_CUDA(cudaMemcpyAsync(parts.data(), nin_dev, fp_calls * 8, cudaMemcpyDeviceToHost, nullptr));
     if (nd > 0) {
         if (F_rep_host) {
             gather_F_kernel<<<(unsigned)((nd + 255) / 256), 256>>>((unsigned long long)nd, (const int64_t*)rep.p, (const double*)F.p, (double*)Frep.p);
@@ -284,6 +315,9 @@ int u1gf_pipeline_host(const u1gf_orbit* o, uint64_t seed, uint64_t first_start,
     }
     U1GF_CUDA(cudaDeviceSynchronize());
     drain.done = true;
+    int64_t n_in = 0;
+    for (int64_t part : parts) n_in += part;
+    *n_in_region_host = n_in;
     t_launches = launches;
     return U1GF_OK;
 }

@@ -111,6 +111,9 @@ struct u1gf_orbit {
     std::vector<double2> U_lanes_host;  // host copy of the links part of that table (kernel parameter of the NB == 1 kernels)
     // device copy of the links in the row order of the TMA-staged streamed kernel (inside blob), or null
     const double2* U_tma = nullptr;
+    // u1gf_pipeline_host's memory of its last call on this handle: 1 = most starts were their own copy (n_distinct > n/4),
+    // so the next call lets the first pass write the fields of all starts instead of relaxing the representatives again
+    mutable int pipeline_keep_fields = 0;
 };
 
 namespace u1gf {

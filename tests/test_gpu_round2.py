@@ -145,6 +145,46 @@ def test_pipeline_host_equals_separate_calls_and_oracle(b, oracle, ext, seed, n)
     b.lib().u1gf_release_host_scratch()
 
 
+def test_pipeline_host_keeps_fields_on_hot_orbits(b):
+    """A handle remembers that its last u1gf_pipeline_host call found most starts to be their own copy (n_distinct > n/4);
+    the next call then writes the fields of all starts in the first pass and u1gf_check_fp picks the representatives by
+    index, instead of relaxing them a second time.  A start is a pure function of its index, so every output of the two
+    paths is identical; only the number of launches differs.  A cold orbit never takes the second path."""
+    ext, seed, n = (4, 4, 4, 4), 12, 1500
+    orbit = b.Orbit(ext, synth.uniform_links(ext, seed))
+    calls = []
+    for _ in range(3):
+        p = b.pipeline_host(orbit, seed, n, eps=1e-12, nbins=64, first_start=3)
+        calls.append((p, b.last_launch_count()))
+        p = calls[-1][0]
+        calls[-1] = ({k: (np.array(v, copy=True) if isinstance(v, np.ndarray) else v) for k, v in p.items()}, calls[-1][1])
+    (p0, l0), (p1, l1), (p2, l2) = calls
+    assert p0["n_distinct"] > n // 4                       # hot: the first call relaxes the representatives again ...
+    assert l1 < l0 and l2 == l1                            # ... the later ones do not
+    for q in (p1, p2):
+        for k in ("sweeps", "status", "copy_id", "rep", "multiplicity", "region", "hist"):
+            assert (p0[k] == q[k]).all(), k
+        assert p0["n_distinct"] == q["n_distinct"] and p0["n_in_region"] == q["n_in_region"]
+        assert (p0["F_norm"] == q["F_norm"]).all() and (p0["F_rep"] == q["F_rep"]).all()
+        assert np.abs(p0["lambda1"] - q["lambda1"]).max() < 1e-12
+    assert p0["n_in_region"] == int(((p0["region"] & 3) != 0).sum())
+    # a batch of another size on the same handle: the remembered choice carries over, results equal those of a fresh handle
+    fresh = b.Orbit(ext, synth.uniform_links(ext, seed))
+    q, r = b.pipeline_host(orbit, seed, 333, eps=1e-12), None
+    q = {k: (np.array(v, copy=True) if isinstance(v, np.ndarray) else v) for k, v in q.items()}
+    r = b.pipeline_host(fresh, seed, 333, eps=1e-12)
+    assert q["n_distinct"] == r["n_distinct"] and (q["region"] == r["region"]).all() and (q["rep"] == r["rep"]).all()
+    assert np.abs(q["lambda1"] - r["lambda1"]).max() < 1e-12 and q["n_in_region"] == r["n_in_region"]
+    # cold orbit (two copies among 4096 starts): every call takes the re-relaxation path
+    cold = b.Orbit((4, 4), synth.uniform_links((4, 4), 1))
+    counts = []
+    for _ in range(2):
+        c = b.pipeline_host(cold, 1, 4096)
+        counts.append((b.last_launch_count(), c["n_distinct"], c["n_in_region"]))
+    assert counts[0] == counts[1] and counts[0][1] < 1024
+    b.lib().u1gf_release_host_scratch()
+
+
 # ------------------------------------------------------------------------------------------- bias read-out (8(f)-2)
 def test_bias_table_matches_oracle(b, oracle):
     """PAPER.md:L99: over-relaxation "decreases the chance of converging to larger minima and thus introduces a bias".
