@@ -249,7 +249,7 @@ int u1gf_release_host_scratch(void);
  * one lattice per thread block, grid over the samples (L121).
  *   u1gf_create_ensemble   theta_host [n_orbits][V*d] link angles, seeds_host [n_orbits] start seed of each orbit
  *                          (starts of orbit o are those of u1gf_relax_batch with seed seeds[o]).  Only lattice shapes
- *                          with a resident kernel (4x4, 8x8, 4^3, 2^4, 4^4), else U1GF_EINVAL.  Synchronous.
+ *                          with a resident kernel (4x4, 8x8, 10x10, 4^3, 6^3, 2^4, 4^4), else U1GF_EINVAL.  Synchronous.
  *   u1gf_ensemble_orbit    member k as an ordinary orbit handle (owned by the ensemble): for u1gf_check_fp and for
  *                          re-relaxing an orbit's representatives with u1gf_relax_batch(start_ids, g_canon)
  *   u1gf_relax_ensemble    every orbit runs the starts first_start + [0, n_starts_per_orbit); result k of orbit o is at

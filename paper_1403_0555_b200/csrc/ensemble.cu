@@ -51,7 +51,7 @@ int u1gf_create_ensemble(int d, const int32_t* extents, int32_t n_orbits, const 
     const u1gf_orbit* o0 = e->orbits[0];
     if (!lanes_supported(o0)) {
         u1gf_destroy_ensemble(e);
-        return fail(U1GF_EINVAL, "u1gf_create_ensemble: no resident kernel for these extents (4x4, 8x8, 4^3, 2^4, 4^4 have one)");
+        return fail(U1GF_EINVAL, "u1gf_create_ensemble: no resident kernel for these extents (4x4, 8x8, 10x10, 4^3, 6^3, 2^4, 4^4 have one)");
     }
     const size_t tab_bytes = lanes_links_bytes(o0->dev.d, o0->dev.ext);
     e->lanes_stride = tab_bytes / sizeof(double2);
