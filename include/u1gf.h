@@ -41,7 +41,8 @@ typedef struct u1gf_orbit u1gf_orbit; /* opaque, library-owned */
 
 const char* u1gf_last_error(void);
 
-/* Version of this ABI (bumped on incompatible change; 2 = round 2: ensembles, pipeline, region bit 2). */
+/* Version of this ABI (2 = round 2: ensembles, pipeline, region bit 2; 3 = round 3: u1gf_paper_count_static and the
+ * ensemble read-outs added, nothing removed or changed). */
 int u1gf_abi_version(void);
 
 /* ---------------------------------------------------------------------------------------------------------
@@ -276,6 +277,46 @@ int u1gf_count_copies_ensemble(int32_t n_orbits, uint64_t n_per_orbit, const dou
                                const uint8_t* status, double tol_F, double tol_sig, int32_t* copy_id,
                                int64_t* n_distinct, int64_t* rep, int64_t* multiplicity, int64_t* hist, int32_t nbins,
                                void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Ensemble read-outs: the quantities the paper tabulates and plots from an ensemble of orbits.
+ * Inputs are the device arrays of u1gf_relax_ensemble / u1gf_count_copies_ensemble: F_norm [n_orbits*n_per_orbit],
+ * rep / multiplicity [n_orbits*n_per_orbit] (entries c < n_distinct[o] of orbit o at o*n_per_orbit + c, rep local to the
+ * orbit), n_distinct [n_orbits].  The paper's value of a minimum is x = 1 - F/(dV) (Eq. 3); its
+ * "global minimum" of an orbit is the smallest x found there, x_g = 1 - max_c F_norm[rep[c]] (L169: "the smallest minimum
+ * we find on each orbit").  All three calls are asynchronous on the stream, need no workspace and allocate nothing.
+ *
+ * u1gf_ensemble_stats     best_x dev [n_orbits]: x_g per orbit (NaN for an orbit without a converged start).
+ *                         stats dev [8]: [0],[1] average and standard deviation over the orbits of n_distinct (Tab. I,
+ *                         PAPER.md:L175-183); [2],[3] of x_g (Tab. III; orbits with NaN left out); [4],[5] of
+ *                         n_in_region (dev [n_orbits] int64: copies inside the first Gribov region per orbit, L9/L50; NULL:
+ *                         NaN); [6] orbits that entered [2],[3]; [7] n_orbits.  Standard deviation = sqrt(sum (v-mean)^2 /
+ *                         (m-1)), 0 for m = 1 (reading R18: the paper prints "avg +- std" without a formula); sums run in
+ *                         orbit order.
+ * u1gf_relative_deviation_hist   (x_i - x_g)/x_g of every converged sample (Fig. 8): copy c of orbit o
+ *                         puts multiplicity[c] samples into bin floor(dev / (dev_max/nbins)) of nbins equal bins on
+ *                         [0, dev_max), larger values into the last bin.  counts dev [n_orbits*nbins] int64 per orbit;
+ *                         n_converged dev [n_orbits] int64 = samples binned; avg dev [nbins] = the orbit average of
+ *                         counts[o][b]/n_converged[o] ("subsequently, the data has been averaged over all orbits", L207)
+ *                         over the n_orbits_used dev [1] orbits that have samples and x_g > 0 (the trivial orbit, x_g = 0,
+ *                         has no relative deviation).  best_x: as written by u1gf_ensemble_stats.
+ * u1gf_hist_ratio         ratio[b] = hist_big[b] / hist_small[b] for two histograms (int64 [nbins], e.g. `hist` of
+ *                         u1gf_count_copies) of the same orbits from a larger and a smaller number of samples (PAPER.md:L167,
+ *                         Fig. 5: 256 against 4 mebisamples in bins of 1e-4): +inf where only the larger run has entries,
+ *                         NaN where neither has; n_only dev [2] int64 = number of bins only the larger / only the smaller
+ *                         run fills (L167: "only very high-lying bins of the four mebisample run are empty while the
+ *                         corresponding bins of the 256 mebisample run have entries").
+ * Errors: U1GF_EINVAL on NULL arrays or sizes < 1, U1GF_ENODEV, U1GF_ECUDA.
+ * ------------------------------------------------------------------------------------------------------- */
+int u1gf_ensemble_stats(int32_t n_orbits, uint64_t n_per_orbit, const double* F_norm, const int64_t* rep,
+                        const int64_t* n_distinct, const int64_t* n_in_region, double* best_x, double* stats,
+                        void* cuda_stream);
+int u1gf_relative_deviation_hist(int32_t n_orbits, uint64_t n_per_orbit, const double* F_norm, const int64_t* rep,
+                                 const int64_t* multiplicity, const int64_t* n_distinct, const double* best_x, double dev_max,
+                                 int32_t nbins, int64_t* counts, int64_t* n_converged, double* avg, int64_t* n_orbits_used,
+                                 void* cuda_stream);
+int u1gf_hist_ratio(int32_t nbins, const int64_t* hist_small, const int64_t* hist_big, double* ratio, int64_t* n_only,
+                    void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------------------
  * Merging the copy tables of several start ranges (the paper runs 4 GPUs on independent samples,

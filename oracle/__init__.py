@@ -286,3 +286,92 @@ def paper_count(F_norm, status, scale=1e8):
             keys.add(int(np.floor((1.0 - float(f)) * float(scale))))
     return len(keys)
 
+
+
+# ------------------------------------------------------------------------------------------------
+# Ensemble read-outs: what the paper tabulates / plots from many orbits.  Plain loops.
+# Per orbit the inputs are the outputs of count_copies on that orbit: F_rep[c] (F/(dV) of the leader of
+# copy c) and multiplicity[c].  The paper's value of a minimum is x = 1 - F/(dV) (Eq. 3).
+# ------------------------------------------------------------------------------------------------
+def _mean_std(values):
+    """Average and standard deviation as printed in Tab. I / III ("avg +- std"; the paper gives no formula --
+    reading R18: sample standard deviation, n-1 in the denominator, 0 for one value), NaN entries left out."""
+    v = [float(x) for x in values if not np.isnan(x)]
+    if not v:
+        return float("nan"), float("nan")
+    s = 0.0
+    for x in v:
+        s = s + x
+    mean = s / len(v)
+    q = 0.0
+    for x in v:
+        e = x - mean
+        q = q + e * e
+    return mean, (float(np.sqrt(q / (len(v) - 1))) if len(v) > 1 else 0.0)
+
+
+def ensemble_stats(F_rep_per_orbit, n_in_region=None):
+    """Tab. I (PAPER.md:L175-183): average and standard deviation over the orbits of the number of distinct minima;
+    Tab. III (L213-220): of the value at the global minimum, x_g = the smallest x found on the orbit (L169) =
+    1 - max_c F_rep[c]; and of the number of copies inside the first Gribov region (L9, L50) when given.
+    Returns dict(best_x [n_orbits], n_distinct=(mean, std), best=(mean, std), n_in_region=(mean, std), used)."""
+    best = []
+    for F in F_rep_per_orbit:
+        F = np.asarray(F, dtype=np.float64)
+        best.append(1.0 - float(F.max()) if F.size else float("nan"))
+    nd = [float(np.asarray(F).size) for F in F_rep_per_orbit]
+    return dict(best_x=np.array(best), n_distinct=_mean_std(nd), best=_mean_std(best),
+                n_in_region=_mean_std([float(v) for v in n_in_region]) if n_in_region is not None else (float("nan"),) * 2,
+                used=sum(1 for b in best if not np.isnan(b)))
+
+
+def relative_deviation_hist(F_rep_per_orbit, multiplicity_per_orbit, dev_max, nbins):
+    """Fig. 8: "the distribution of the minima F_i relative to the global minimum F_g on that
+    orbit: (F_i - F_g)/F_g.  Subsequently, the data has been averaged over all orbits."  In the paper's convention the
+    F there are the values x.  Every converged sample counts (a copy found m times puts m entries: the bins of Fig. 5
+    scale with the number of samples, L167 -- reading R19).  nbins equal bins on [0, dev_max), larger values in the
+    last bin.  Orbits without samples or with x_g = 0 (trivial orbit: no relative deviation) are left out.
+    Returns dict(counts [n_orbits, nbins], n_converged [n_orbits], avg [nbins], used)."""
+    n_orb = len(F_rep_per_orbit)
+    counts = np.zeros((n_orb, nbins), dtype=np.int64)
+    nconv = np.zeros(n_orb, dtype=np.int64)
+    width = float(dev_max) / float(nbins)
+    for o in range(n_orb):
+        F = np.asarray(F_rep_per_orbit[o], dtype=np.float64)
+        m = np.asarray(multiplicity_per_orbit[o], dtype=np.int64)
+        if F.size == 0:
+            continue
+        xg = 1.0 - float(F.max())
+        if not xg > 0.0:
+            continue
+        for c in range(F.size):
+            x = 1.0 - float(F[c])
+            dev = (x - xg) / xg
+            q = int(np.floor(dev / width))
+            b = 0 if q < 0 else (nbins - 1 if q >= nbins else q)
+            counts[o, b] += int(m[c])
+            nconv[o] += int(m[c])
+    avg = np.zeros(nbins)
+    used = 0
+    for b in range(nbins):
+        s, used = 0.0, 0
+        for o in range(n_orb):
+            if nconv[o] == 0:
+                continue
+            s = s + float(counts[o, b]) / float(nconv[o])
+            used += 1
+        avg[b] = s / used if used else 0.0
+    return dict(counts=counts, n_converged=nconv, avg=avg, used=used)
+
+
+def hist_ratio(hist_small, hist_big):
+    """Fig. 5: "We assign each minimum to a bin of resolution 1e-4 and plot the ratios of the
+    entries of the bins from 256 vs. four mebisamples"; "only very high-lying bins of the four mebisample run are empty
+    while the corresponding bins of the 256 mebisample run have entries".  ratio[b] = big/small (inf where only the
+    larger run has entries, NaN where neither); n_only = (bins only the larger run fills, bins only the smaller)."""
+    ratio, only_big, only_small = [], 0, 0
+    for s, g in zip(np.asarray(hist_small).tolist(), np.asarray(hist_big).tolist()):
+        ratio.append(g / s if s > 0 else (float("inf") if g > 0 else float("nan")))
+        only_big += 1 if (s == 0 and g > 0) else 0
+        only_small += 1 if (g == 0 and s > 0) else 0
+    return dict(ratio=np.array(ratio), n_only=(only_big, only_small))

@@ -54,6 +54,10 @@ _SIGNATURES = {
     "u1gf_count_ensemble_workspace_bytes": (C.c_size_t, [C.c_uint64]),
     "u1gf_count_copies_ensemble": (C.c_int, [C.c_int32, C.c_uint64, _p, _p, _p, C.c_double, C.c_double, _p, _p, _p, _p, _p,
                                              C.c_int32, _p, C.c_size_t, _p]),
+    "u1gf_ensemble_stats": (C.c_int, [C.c_int32, C.c_uint64, _p, _p, _p, _p, _p, _p, _p]),
+    "u1gf_relative_deviation_hist": (C.c_int, [C.c_int32, C.c_uint64, _p, _p, _p, _p, _p, C.c_double, C.c_int32, _p, _p, _p,
+                                               _p, _p]),
+    "u1gf_hist_ratio": (C.c_int, [C.c_int32, _p, _p, _p, _p, _p]),
     "u1gf_merge_workspace_bytes": (C.c_size_t, [C.c_uint64]),
     "u1gf_merge_copy_tables": (C.c_int, [C.c_uint64, _p, _p, _p, _p, C.c_double, C.c_double, _p, _p, _p, _p, _p,
                                          C.c_size_t, _p]),
@@ -269,6 +273,41 @@ def merge_copy_tables(F_rep, sig_rep, first_start, multiplicity, tol_F=1e-10, to
                                         float(tol_F), float(tol_sig), _dev_ptr(mid), _dev_ptr(nm), _dev_ptr(mfs),
                                         _dev_ptr(mmu), _aligned_ptr(ws), need, _stream()))
     return dict(merged_id=mid, n_merged=nm, first_start=mfs, multiplicity=mmu)
+
+
+def ensemble_stats(n_orbits, n_per_orbit, F_norm, rep, n_distinct, n_in_region=None):
+    """u1gf_ensemble_stats on the device arrays of relax_ensemble / count_copies_ensemble -> dict(best_x [n_orbits], stats [8])."""
+    import torch
+    best = torch.empty(int(n_orbits), dtype=torch.float64, device="cuda")
+    stats = torch.empty(8, dtype=torch.float64, device="cuda")
+    _check(lib().u1gf_ensemble_stats(int(n_orbits), int(n_per_orbit), _dev_ptr(F_norm), _dev_ptr(rep), _dev_ptr(n_distinct),
+                                     _dev_ptr(n_in_region), _dev_ptr(best), _dev_ptr(stats), _stream()))
+    return dict(best_x=best, stats=stats)
+
+
+def relative_deviation_hist(n_orbits, n_per_orbit, F_norm, rep, multiplicity, n_distinct, best_x, dev_max, nbins):
+    """u1gf_relative_deviation_hist -> dict(counts [n_orbits, nbins], n_converged [n_orbits], avg [nbins], n_orbits_used [1])."""
+    import torch
+    counts = torch.empty((int(n_orbits), int(nbins)), dtype=torch.int64, device="cuda")
+    nconv = torch.empty(int(n_orbits), dtype=torch.int64, device="cuda")
+    avg = torch.empty(int(nbins), dtype=torch.float64, device="cuda")
+    used = torch.empty(1, dtype=torch.int64, device="cuda")
+    _check(lib().u1gf_relative_deviation_hist(int(n_orbits), int(n_per_orbit), _dev_ptr(F_norm), _dev_ptr(rep),
+                                              _dev_ptr(multiplicity), _dev_ptr(n_distinct), _dev_ptr(best_x), float(dev_max),
+                                              int(nbins), _dev_ptr(counts), _dev_ptr(nconv), _dev_ptr(avg), _dev_ptr(used),
+                                              _stream()))
+    return dict(counts=counts, n_converged=nconv, avg=avg, n_orbits_used=used)
+
+
+def hist_ratio(hist_small, hist_big):
+    """u1gf_hist_ratio on two device int64 histograms -> dict(ratio [nbins], n_only [2])."""
+    import torch
+    nb = int(hist_small.numel())
+    assert int(hist_big.numel()) == nb
+    ratio = torch.empty(nb, dtype=torch.float64, device="cuda")
+    n_only = torch.empty(2, dtype=torch.int64, device="cuda")
+    _check(lib().u1gf_hist_ratio(nb, _dev_ptr(hist_small), _dev_ptr(hist_big), _dev_ptr(ratio), _dev_ptr(n_only), _stream()))
+    return dict(ratio=ratio, n_only=n_only)
 
 
 def pipeline_host(orbit, seed, n_starts, *, first_start=0, omega=1.7, eps=1e-13, max_sweeps=20000, check_every=1,

@@ -18,7 +18,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libu1gf.so")                   # the method: include/u1gf.h
 LIB_MEASURE = os.path.join(HERE, "libu1gf_measure.so")   # roofline probes: include/u1gf_measure.h (not the method)
 SOURCES = ["common.cu", "orbit.cu", "relax_generic.cu", "relax_lanes.cu", "relax_stream.cu", "relax_tma.cu", "count_copies.cu",
-           "discovery.cu", "check_fp.cu", "host_calls.cu", "ensemble.cu", "merge.cu"]
+           "discovery.cu", "check_fp.cu", "host_calls.cu", "ensemble.cu", "merge.cu", "readout.cu"]
 MEASURE_SOURCES = [("common.cu", "common_measure.o", ["-DU1GF_MEASURE_LIB"]), ("peaks.cu", "peaks.o", [])]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]

@@ -59,7 +59,7 @@ extern "C" {
 const char* u1gf_measure_last_error(void) { return t_err; }
 #else
 const char* u1gf_last_error(void) { return t_err; }
-int u1gf_abi_version(void) { return 2; }
+int u1gf_abi_version(void) { return 3; }
 int32_t u1gf_last_launch_count(void) { return t_launches; }
 #endif
 

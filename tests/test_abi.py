@@ -31,7 +31,7 @@ def test_header_symbols_are_exported_and_bound(binding):
     for name in declared:
         assert hasattr(L, name), f"{name} declared in include/u1gf.h but not exported by libu1gf.so"
     assert declared == binding.exported_symbols(), "binding._SIGNATURES must list exactly the header's symbols"
-    assert binding.lib().u1gf_abi_version() == 2
+    assert binding.lib().u1gf_abi_version() == 3
     # the method's header carries no measurement or debug entry points; those live in include/u1gf_measure.h
     assert not [n for n in declared if "measure" in n or n.startswith("u1gf_last_") and n != "u1gf_last_error"]
 

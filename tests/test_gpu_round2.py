@@ -72,6 +72,78 @@ def test_ensemble_one_launch_matches_single_orbits_and_oracle(b, oracle, ext, se
     torch.cuda.synchronize()
 
 
+def test_ensemble_readouts_match_oracle(b, oracle):
+    """u1gf_ensemble_stats / u1gf_relative_deviation_hist / u1gf_hist_ratio (Tab. I, Tab. III, Fig. 8, Fig. 5 of the paper)
+    on ensembles relaxed and de-duplicated on the device, against the oracle's definitions on the same copy tables:
+    integer outputs bit for bit, floating-point outputs within 1e-10; and x_g, n_distinct also against the oracle's own
+    relaxation of every orbit."""
+    import torch
+    for ext, seeds, n, dev_max, nbins in (((4, 4), list(range(1, 13)), 2048, 0.6, 48), ((4, 4, 4), [3, 4, 5, 6], 3000, 0.25, 1000),
+                                          ((2, 2, 2, 2), [12, 13, 14], 500, 0.5, 7)):
+        thetas = [synth.uniform_links(ext, s) for s in seeds]
+        ens = b.Ensemble(ext, np.stack(thetas), seeds)
+        r = b.relax_ensemble(ens, n)
+        c = b.count_copies_ensemble(r["F_norm"], r["sig"], r["status"], nbins=10000)
+        K = len(seeds)
+        nds = _cpu(c["n_distinct"])
+        Fg, rep, mul = _cpu(r["F_norm"]), _cpu(c["rep"]), _cpu(c["multiplicity"])
+        F_rep = [Fg[k][rep[k][:nds[k]]] for k in range(K)]
+        mult = [mul[k][:nds[k]] for k in range(K)]
+        n_in = torch.tensor([(7 * k + 3) % 5 for k in range(K)], dtype=torch.int64, device="cuda")   # any integers do here
+        s = b.ensemble_stats(K, n, r["F_norm"], c["rep"], c["n_distinct"], n_in)
+        os_ = oracle.ensemble_stats(F_rep, n_in_region=_cpu(n_in))
+        best, stats = _cpu(s["best_x"]), _cpu(s["stats"])
+        assert (best == os_["best_x"]).all()                        # one exact subtraction from the same F
+        want = [*os_["n_distinct"], *os_["best"], *os_["n_in_region"], os_["used"], K]
+        assert np.abs(stats - np.array(want, dtype=np.float64)).max() < 1e-10
+        s0 = _cpu(b.ensemble_stats(K, n, r["F_norm"], c["rep"], c["n_distinct"])["stats"])
+        assert np.isnan(s0[4]) and np.isnan(s0[5]) and (s0[:4] == stats[:4]).all()
+        # against the oracle's own relaxation: same number of copies, same best value per orbit
+        for k in range(K):
+            o = oracle.relax(ext, thetas[k], seeds[k], n)
+            oc = oracle.count_copies(o["F_norm"], o["sig"], o["status"])
+            assert oc["n_distinct"] == nds[k] and abs((1.0 - oc["F_rep"].max()) - best[k]) < TOL_F
+        d = b.relative_deviation_hist(K, n, r["F_norm"], c["rep"], c["multiplicity"], c["n_distinct"], s["best_x"], dev_max, nbins)
+        od = oracle.relative_deviation_hist(F_rep, mult, dev_max, nbins)
+        assert (_cpu(d["counts"]) == od["counts"]).all() and (_cpu(d["n_converged"]) == od["n_converged"]).all()
+        assert int(d["n_orbits_used"].item()) == od["used"] == K
+        assert np.abs(_cpu(d["avg"]) - od["avg"]).max() < 1e-10 and abs(_cpu(d["avg"]).sum() - 1.0) < 1e-12
+        assert (_cpu(d["n_converged"]) == n).all()                  # every start converged: every sample is binned
+        # Fig. 5: the same orbits with a quarter of the samples (the first n/4 starts of each orbit are a prefix)
+        r4 = b.relax_ensemble(ens, n // 4)
+        c4 = b.count_copies_ensemble(r4["F_norm"], r4["sig"], r4["status"], nbins=10000)
+        big, small = c["hist"].sum(dim=0), c4["hist"].sum(dim=0)
+        h = b.hist_ratio(small, big)
+        oh = oracle.hist_ratio(_cpu(small), _cpu(big))
+        ratio = _cpu(h["ratio"])
+        assert np.array_equal(np.isnan(ratio), np.isnan(oh["ratio"])) and np.array_equal(np.isinf(ratio), np.isinf(oh["ratio"]))
+        fin = np.isfinite(ratio)
+        assert (ratio[fin] == oh["ratio"][fin]).all() and tuple(_cpu(h["n_only"]).tolist()) == oh["n_only"]
+        assert oh["n_only"][1] == 0                                 # a prefix of the samples cannot fill a bin the full run misses
+        ens.close()
+    # an orbit without a converged start and the trivial orbit: NaN / left out, as the oracle does
+    ext = (4, 4)
+    th = np.stack([synth.uniform_links(ext, 1), synth.cold_links(ext)])
+    ens = b.Ensemble(ext, th, [1, 2])
+    r = b.relax_ensemble(ens, 256)
+    c = b.count_copies_ensemble(r["F_norm"], r["sig"], r["status"])
+    s = b.ensemble_stats(2, 256, r["F_norm"], c["rep"], c["n_distinct"])
+    d = b.relative_deviation_hist(2, 256, r["F_norm"], c["rep"], c["multiplicity"], c["n_distinct"], s["best_x"], 1.0, 10)
+    nds = _cpu(c["n_distinct"])
+    Fg, rep, mul = _cpu(r["F_norm"]), _cpu(c["rep"]), _cpu(c["multiplicity"])
+    od = oracle.relative_deviation_hist([Fg[k][rep[k][:nds[k]]] for k in range(2)], [mul[k][:nds[k]] for k in range(2)], 1.0, 10)
+    assert (_cpu(d["counts"]) == od["counts"]).all() and int(d["n_orbits_used"].item()) == od["used"]
+    assert np.abs(_cpu(d["avg"]) - od["avg"]).max() < 1e-10
+    st2 = r["status"].clone()
+    st2[1] |= 1                                                     # orbit 1: nothing converged
+    c2 = b.count_copies_ensemble(r["F_norm"], r["sig"], st2)
+    s2 = b.ensemble_stats(2, 256, r["F_norm"], c2["rep"], c2["n_distinct"])
+    assert np.isnan(_cpu(s2["best_x"])[1]) and _cpu(s2["stats"])[6] == 1.0 and _cpu(s2["stats"])[3] == 0.0
+    ens.close()
+    with pytest.raises(b.U1gfError):
+        b.hist_ratio(torch.zeros(0, dtype=torch.int64, device="cuda"), torch.zeros(0, dtype=torch.int64, device="cuda"))
+
+
 # ------------------------------------------------------------------------------------------- table merge (8(f)-4)
 @pytest.mark.parametrize("ext,seed,n,cuts", [((4, 4, 4), 3, 20000, (0, 7000, 7001, 20000)), ((4, 4), 1, 4096, (0, 2048, 4096)),
                                              ((4, 4, 4, 4), 12, 3000, (0, 1000, 2000, 3000))])

@@ -529,3 +529,39 @@ def test_discovery_curve_and_paper_count_pins(oracle):
     sg = np.array([[.1, .2, .3, .4], [-.3, .2, .1, 0.]])
     assert oracle.count_copies(Fc, sg, np.zeros(2, np.uint8))["n_distinct"] == 2
     assert oracle.paper_count(Fc, np.zeros(2, np.uint8)) == 1
+
+
+def test_ensemble_readout_pins(oracle):
+    """SURVEY 8(f)-3 read-outs on hand-made copy tables whose answers are worked out by hand (binary fractions, so
+    every value below is exact in FP64)."""
+    # three orbits: best F/(dV) 0.75, 0.5, 0.875 -> x_g 0.25, 0.5, 0.125; copies 3, 1, 2
+    Fs = [np.array([0.5, 0.75, 0.25]), np.array([0.5]), np.array([0.875, 0.75])]
+    ms = [np.array([2, 5, 1]), np.array([4]), np.array([1, 3])]
+    st = oracle.ensemble_stats(Fs, n_in_region=[3, 1, 0])
+    assert st["best_x"].tolist() == [0.25, 0.5, 0.125]
+    assert st["n_distinct"] == (2.0, 1.0)                      # mean of 3,1,2; sqrt(((1)^2+(1)^2+0)/2) = 1
+    assert st["best"][0] == 0.875 / 3 and abs(st["best"][1] - np.std([0.25, 0.5, 0.125], ddof=1)) < 1e-15
+    assert st["n_in_region"][0] == 4.0 / 3 and abs(st["n_in_region"][1] - np.std([3, 1, 0], ddof=1)) < 1e-15
+    assert st["used"] == 3
+    # one orbit: standard deviation 0; an orbit without copies is NaN and left out of the x_g average
+    assert oracle.ensemble_stats([np.array([0.5])])["n_distinct"] == (1.0, 0.0)
+    s2 = oracle.ensemble_stats([np.array([0.5]), np.zeros(0)])
+    assert np.isnan(s2["best_x"][1]) and s2["best"] == (0.5, 0.0) and s2["used"] == 1 and s2["n_distinct"][0] == 0.5
+    # relative deviation (x_i - x_g)/x_g.  Orbit 0: x = 0.5, 0.25, 0.75 with x_g 0.25 -> dev 1, 0, 2 (weights 2, 5, 1);
+    # orbit 1: dev 0 (weight 4); orbit 2: x = 0.125, 0.25 -> dev 0, 1 (weights 1, 3).  4 bins on [0, 2): width 0.5
+    r = oracle.relative_deviation_hist(Fs, ms, dev_max=2.0, nbins=4)
+    assert r["counts"].tolist() == [[5, 0, 2, 1], [4, 0, 0, 0], [1, 0, 3, 0]]      # dev 2 >= dev_max: last bin
+    assert r["n_converged"].tolist() == [8, 4, 4] and r["used"] == 3
+    assert np.allclose(r["avg"], [(5 / 8 + 1 + 1 / 4) / 3, 0, (2 / 8 + 3 / 4) / 3, (1 / 8) / 3], rtol=0, atol=1e-16)
+    assert abs(r["avg"].sum() - 1.0) < 1e-15                    # fractions of samples: the average sums to one
+    # the trivial orbit (F/(dV) = 1, x_g = 0) and an empty orbit are left out
+    r2 = oracle.relative_deviation_hist([np.array([1.0, 0.5]), np.zeros(0), np.array([0.5, 0.25])],
+                                        [np.array([3, 1]), np.zeros(0, np.int64), np.array([1, 1])], dev_max=1.0, nbins=2)
+    assert r2["counts"].tolist() == [[0, 0], [0, 0], [1, 1]] and r2["used"] == 1 and r2["avg"].tolist() == [0.5, 0.5]
+    # scale invariance: the same copies with every multiplicity times 64 give the same averaged distribution
+    r3 = oracle.relative_deviation_hist(Fs, [64 * m for m in ms], dev_max=2.0, nbins=4)
+    assert (r3["avg"] == r["avg"]).all() and (r3["counts"] == 64 * r["counts"]).all()
+    # Fig. 5 ratios: 64 times the samples in every bin but the last two
+    h = oracle.hist_ratio(np.array([2, 0, 5, 0, 3]), np.array([128, 0, 320, 7, 0]))
+    assert h["ratio"][0] == 64.0 and np.isnan(h["ratio"][1]) and h["ratio"][2] == 64.0 and np.isinf(h["ratio"][3])
+    assert h["ratio"][4] == 0.0 and h["n_only"] == (1, 1)
