@@ -249,15 +249,19 @@ int u1gf_release_host_scratch(void);
  * workload is an ensemble -- 100 orbits x 4 mebisamples per lattice size (Tab. I, Tab. III),
  * one lattice per thread block, grid over the samples (L121).
  *   u1gf_create_ensemble   theta_host [n_orbits][V*d] link angles, seeds_host [n_orbits] start seed of each orbit
- *                          (starts of orbit o are those of u1gf_relax_batch with seed seeds[o]).  Only lattice shapes
- *                          with a resident kernel (4x4, 8x8, 10x10, 4^3, 6^3, 2^4, 4^4), else U1GF_EINVAL.  Synchronous.
+ *                          (starts of orbit o are those of u1gf_relax_batch with seed seeds[o]).  Any lattice
+ *                          u1gf_create_orbit accepts: shapes with a resident kernel (4x4, 8x8, 10x10, 4^3, 6^3, 2^4, 4^4)
+ *                          run on it; every other shape (2x2, 6x6, 2^3, 8^3 of Tab. I / III, odd extents, ...) runs on
+ *                          the generic kernel, one thread block per start with the grid over the starts of all orbits
+ *                          (the paper's own mapping).  Synchronous.
  *   u1gf_ensemble_orbit    member k as an ordinary orbit handle (owned by the ensemble): for u1gf_check_fp and for
  *                          re-relaxing an orbit's representatives with u1gf_relax_batch(start_ids, g_canon)
  *   u1gf_relax_ensemble    every orbit runs the starts first_start + [0, n_starts_per_orbit); result k of orbit o is at
  *                          o * n_starts_per_orbit + k of F_norm / sweeps / status / sig [.*4] (device arrays of
  *                          n_orbits * n_starts_per_orbit entries).  Per start the results are those of
- *                          u1gf_relax_batch on the member orbit, with one exception: a start that meets R6
- *                          (|w|^2 < 1e-280) comes back with status 3 instead of being relaxed with the skip rule.
+ *                          u1gf_relax_batch on the member orbit, with one exception on the shapes with a resident
+ *                          kernel: a start that meets R6 (|w|^2 < 1e-280) comes back with status 3 instead of being
+ *                          relaxed with the skip rule (the generic kernel applies the skip rule as always).
  *   u1gf_count_copies_ensemble   u1gf_count_copies per orbit on those arrays: copy ids, rep (positions) and
  *                          multiplicity are local to the orbit and stored at o * n_per_orbit; n_distinct dev
  *                          [n_orbits]; hist dev [n_orbits * nbins] or NULL; workspace >= u1gf_count_workspace_bytes(n_per_orbit)

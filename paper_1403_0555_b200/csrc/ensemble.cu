@@ -4,6 +4,8 @@
 // (relax_lanes.cu) number their 32-start batches over all orbits of the ensemble; a team of 32 lanes works through its
 // batches orbit by orbit and reloads the link table in shared memory at an orbit boundary.  De-duplication is per
 // orbit (copies of different orbits are unrelated), as a loop over u1gf_count_copies on the orbits' slices.
+// Shapes without a resident kernel (2x2, 6x6, 2^3, 8^3, odd extents, ...) run on the generic kernel, one CTA per start
+// with the grid over the starts of all orbits -- the paper's own mapping.
 #include <new>
 
 #include "u1gf_internal.h"
@@ -14,6 +16,8 @@ struct u1gf_ensemble {
     const double2* U_all = nullptr;
     const unsigned long long* seeds_dev = nullptr;
     unsigned long long lanes_stride = 0;        // double2 elements per orbit
+    bool generic = false;                       // no resident kernel for the shape: plain link tables [V*d] per orbit and
+                                                // the generic kernel, one CTA per start (the paper's mapping, L121)
 };
 
 using namespace u1gf;
@@ -49,11 +53,8 @@ int u1gf_create_ensemble(int d, const int32_t* extents, int32_t n_orbits, const 
         Vd = (size_t)o->dev.V * (size_t)o->dev.d;
     }
     const u1gf_orbit* o0 = e->orbits[0];
-    if (!lanes_supported(o0)) {
-        u1gf_destroy_ensemble(e);
-        return fail(U1GF_EINVAL, "u1gf_create_ensemble: no resident kernel for these extents (4x4, 8x8, 10x10, 4^3, 6^3, 2^4, 4^4 have one)");
-    }
-    const size_t tab_bytes = lanes_links_bytes(o0->dev.d, o0->dev.ext);
+    e->generic = !lanes_supported(o0);
+    const size_t tab_bytes = e->generic ? Vd * sizeof(double2) : lanes_links_bytes(o0->dev.d, o0->dev.ext);
     e->lanes_stride = tab_bytes / sizeof(double2);
     const size_t seeds_off = ((size_t)n_orbits * tab_bytes + 255) & ~(size_t)255;
     cudaError_t err = cudaMalloc(&e->blob, seeds_off + (size_t)n_orbits * sizeof(uint64_t));
@@ -64,7 +65,9 @@ int u1gf_create_ensemble(int d, const int32_t* extents, int32_t n_orbits, const 
     e->U_all = (const double2*)e->blob;
     e->seeds_dev = (const unsigned long long*)((char*)e->blob + seeds_off);
     for (int k = 0; k < n_orbits && err == cudaSuccess; ++k)   // the members' tables, device to device
-        err = cudaMemcpy((char*)e->blob + (size_t)k * tab_bytes, e->orbits[k]->U_lanes, tab_bytes, cudaMemcpyDeviceToDevice);
+        err = cudaMemcpy((char*)e->blob + (size_t)k * tab_bytes,
+                         e->generic ? (const void*)e->orbits[k]->dev.U : (const void*)e->orbits[k]->U_lanes, tab_bytes,
+                         cudaMemcpyDeviceToDevice);
     if (err == cudaSuccess)
         err = cudaMemcpy((char*)e->blob + seeds_off, seeds_host, (size_t)n_orbits * sizeof(uint64_t), cudaMemcpyHostToDevice);
     if (err != cudaSuccess) {
@@ -84,6 +87,7 @@ const u1gf_orbit* u1gf_ensemble_orbit(const u1gf_ensemble* e, int32_t k) {
 
 size_t u1gf_relax_ensemble_workspace_bytes(const u1gf_ensemble* e, uint64_t n_starts_per_orbit) {
     if (!e) return 0;
+    if (e->generic) return generic_workspace_bytes(e->orbits[0], n_starts_per_orbit);
     return lanes_ens_workspace_bytes(e->orbits[0], (unsigned)e->orbits.size(), n_starts_per_orbit);
 }
 
@@ -106,6 +110,8 @@ int u1gf_relax_ensemble(const u1gf_ensemble* e, uint64_t first_start, uint64_t n
     if (((uintptr_t)workspace & 255) != 0) return fail(U1GF_EINVAL, "u1gf_relax_ensemble: workspace not 256-byte aligned");
     RelaxArgs a{0, first_start, n_starts_per_orbit, nullptr, omega, eps, max_sweeps, check_every,
                 F_norm, sweeps, status, sig, nullptr, workspace, workspace_bytes};
+    if (e->generic)
+        return generic_relax_ens(e->orbits[0], e->U_all, e->seeds_dev, (unsigned)e->orbits.size(), a, (cudaStream_t)cuda_stream);
     return lanes_relax_ens(e->orbits[0], e->U_all, e->lanes_stride, e->seeds_dev, (unsigned)e->orbits.size(), a,
                            (cudaStream_t)cuda_stream);
 }

@@ -28,20 +28,26 @@ struct Params {
     // work list is the position pos[idx] in the output arrays (and in start_ids); both NULL otherwise
     const unsigned* n_dev;
     const unsigned long long* pos;
+    // ensemble mode (the paper's own mapping, one lattice per block with the grid over the samples of all
+    // orbits): work item k is start first_start + k % ens_n_per of orbit k / ens_n_per, whose links are at
+    // ens_U + orbit * V * DIM and whose start seed is ens_seeds[orbit]; n_starts = n_orbits * ens_n_per.  NULL otherwise
+    const double2* ens_U;
+    const unsigned long long* ens_seeds;
+    unsigned long long ens_n_per;
 };
 
 // w_i = sum_mu [ conj(U_{i,mu}) g_{i+mu} + U_{i-mu,mu} g_{i-mu} ]   (= conj K_i of Eq. 5)
 template <int DIM>
-__device__ __forceinline__ void neighbour_sum(const OrbitDev& D, const double2* __restrict__ g, int i, double& wr,
-                                              double& wi) {
+__device__ __forceinline__ void neighbour_sum(const OrbitDev& D, const double2* __restrict__ U,
+                                              const double2* __restrict__ g, int i, double& wr, double& wi) {
     wr = 0.0;
     wi = 0.0;
 #pragma unroll
     for (int mu = 0; mu < DIM; ++mu) {
         const int jf = __ldg(D.fwd + i * DIM + mu);
         const int jb = __ldg(D.bwd + i * DIM + mu);
-        const double2 u = __ldg(D.U + i * DIM + mu);
-        const double2 b = __ldg(D.U + jb * DIM + mu);
+        const double2 u = __ldg(U + i * DIM + mu);
+        const double2 b = __ldg(U + jb * DIM + mu);
         const double2 gf = g[jf];
         const double2 gb = g[jb];
         wr = fma(u.x, gf.x, wr);
@@ -110,12 +116,20 @@ __global__ void __launch_bounds__(1024) relax_generic_kernel(const OrbitDev D, c
         unsigned long long k = s_next;
         if (k >= (P.n_dev ? (unsigned long long)*P.n_dev : P.n_starts)) break;
         if (P.pos) k = P.pos[k];
-        const uint64_t s = P.start_ids ? P.start_ids[k] : P.first_start + k;
+        uint64_t s = P.start_ids ? P.start_ids[k] : P.first_start + k;
+        uint64_t seed = P.seed;
+        const double2* __restrict__ U = D.U;
+        if (P.ens_U) {   // the orbit this start belongs to (results stay at position k)
+            const unsigned long long orb = k / P.ens_n_per;
+            s = P.first_start + (k - orb * P.ens_n_per);
+            seed = P.ens_seeds[orb];
+            U = P.ens_U + orb * (unsigned long long)(V * DIM);
+        }
 
         // a2: random start
         for (int i = tid; i < V; i += T) {
-            const u32x4 r = philox((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 0u, (uint32_t)P.seed,
-                                   (uint32_t)(P.seed >> 32));
+            const u32x4 r = philox((uint32_t)i, (uint32_t)s, (uint32_t)(s >> 32), 0u, (uint32_t)seed,
+                                   (uint32_t)(seed >> 32));
             double sn, cs;
             sincospi(unit_interval_pm1(r.x, r.y), &sn, &cs);
             g[i] = make_double2(cs, sn);
@@ -143,7 +157,7 @@ __global__ void __launch_bounds__(1024) relax_generic_kernel(const OrbitDev D, c
                         const int i = __ldg(D.order + q);
                         site[j] = i;
                         double wr, wi;
-                        neighbour_sum<DIM>(D, g, i, wr, wi);
+                        neighbour_sum<DIM>(D, U, g, i, wr, wi);
                         const double2 gi = g[i];
                         const double dl = fma(gi.y, wr, -gi.x * wi);  // Delta_i = Im(g_i conj w_i)
                         accE = fma(dl, dl, accE);
@@ -170,7 +184,7 @@ __global__ void __launch_bounds__(1024) relax_generic_kernel(const OrbitDev D, c
                     if (q < off2) {
                         const int i = __ldg(D.order + q);
                         double wr, wi;
-                        neighbour_sum<DIM>(D, g, i, wr, wi);
+                        neighbour_sum<DIM>(D, U, g, i, wr, wi);
                         const double2 gn = site_update(g[i], wr, wi, P.omega, skipped);
                         g[i] = gn;
                         const double dl = fma(gn.y, wr, -gn.x * wi);
@@ -188,7 +202,7 @@ __global__ void __launch_bounds__(1024) relax_generic_kernel(const OrbitDev D, c
                     for (int q = D.phase_off[p] + tid; q < D.phase_off[p + 1]; q += T) {
                         const int i = __ldg(D.order + q);
                         double wr, wi;
-                        neighbour_sum<DIM>(D, g, i, wr, wi);
+                        neighbour_sum<DIM>(D, U, g, i, wr, wi);
                         g[i] = site_update(g[i], wr, wi, P.omega, skipped);
                     }
                     __syncthreads();
@@ -199,7 +213,7 @@ __global__ void __launch_bounds__(1024) relax_generic_kernel(const OrbitDev D, c
                     double S = 0.0, Fp = 0.0;
                     for (int i = tid; i < V; i += T) {
                         double wr, wi;
-                        neighbour_sum<DIM>(D, g, i, wr, wi);
+                        neighbour_sum<DIM>(D, U, g, i, wr, wi);
                         const double2 gi = g[i];
                         const double dl = fma(gi.y, wr, -gi.x * wi);
                         S = fma(dl, dl, S);
@@ -296,7 +310,7 @@ size_t generic_workspace_bytes(const u1gf_orbit*, uint64_t) { return 256; }
 int generic_relax_list(const u1gf_orbit* o, const RelaxArgs& a, const unsigned* n_dev, const unsigned long long* pos,
                        unsigned long long* counter, cudaStream_t st) {
     Params P{a.seed, a.first_start, a.n_starts, a.start_ids, a.omega, a.eps, a.max_sweeps, a.check_every,
-             a.F_norm, a.sweeps, a.status, a.sig, a.g_canon, counter, n_dev, pos};
+             a.F_norm, a.sweeps, a.status, a.sig, a.g_canon, counter, n_dev, pos, nullptr, nullptr, 0ull};
     // a small grid: the list is empty unless a neighbour sum vanished somewhere (R6)
     if (P.n_starts > 4ull * (unsigned long long)o->sm_count) P.n_starts = 4ull * (unsigned long long)o->sm_count;
     const Launch L = pick(o);
@@ -310,7 +324,23 @@ int generic_relax_list(const u1gf_orbit* o, const RelaxArgs& a, const unsigned* 
 
 int generic_relax(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st) {
     Params P{a.seed, a.first_start, a.n_starts, a.start_ids, a.omega, a.eps, a.max_sweeps, a.check_every,
-             a.F_norm, a.sweeps, a.status, a.sig, a.g_canon, (unsigned long long*)a.workspace, nullptr, nullptr};
+             a.F_norm, a.sweeps, a.status, a.sig, a.g_canon, (unsigned long long*)a.workspace, nullptr, nullptr,
+             nullptr, nullptr, 0ull};
+    const Launch L = pick(o);
+    switch (o->dev.d) {
+        case 1: return launch_d<1>(o, P, L, st);
+        case 2: return launch_d<2>(o, P, L, st);
+        case 3: return launch_d<3>(o, P, L, st);
+        default: return launch_d<4>(o, P, L, st);
+    }
+}
+
+// Ensemble mode: a.n_starts starts of each of n_orbits orbits of the shape of `o` in one launch (a.seed is not used).
+int generic_relax_ens(const u1gf_orbit* o, const double2* U_all, const unsigned long long* seeds, unsigned n_orbits,
+                      const RelaxArgs& a, cudaStream_t st) {
+    Params P{0, a.first_start, a.n_starts * (uint64_t)n_orbits, nullptr, a.omega, a.eps, a.max_sweeps, a.check_every,
+             a.F_norm, a.sweeps, a.status, a.sig, nullptr, (unsigned long long*)a.workspace, nullptr, nullptr,
+             U_all, seeds, (unsigned long long)a.n_starts};
     const Launch L = pick(o);
     switch (o->dev.d) {
         case 1: return launch_d<1>(o, P, L, st);

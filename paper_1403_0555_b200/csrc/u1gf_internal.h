@@ -135,6 +135,9 @@ struct RelaxArgs {
 
 size_t generic_workspace_bytes(const u1gf_orbit* o, uint64_t n);
 int generic_relax(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st);
+// ensemble mode of the same kernel: n_orbits orbits of o's shape, links [n_orbits][V*d] at U_all, a.n_starts starts each
+int generic_relax_ens(const u1gf_orbit* o, const double2* U_all, const unsigned long long* seeds, unsigned n_orbits,
+                      const RelaxArgs& a, cudaStream_t st);
 // redo mode: relax the starts at output positions pos[0 .. *n_dev) again (R6 fix-up of the resident kernels); `counter` is a
 // zeroed device word
 int generic_relax_list(const u1gf_orbit* o, const RelaxArgs& a, const unsigned* n_dev, const unsigned long long* pos,

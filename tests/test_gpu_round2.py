@@ -30,7 +30,11 @@ def _cpu(t):
 # ------------------------------------------------------------------------------------------- ensembles (8(f)-3)
 @pytest.mark.parametrize("ext,seeds,n", [((4, 4, 4), list(range(3, 11)), 4100), ((4, 4), [1, 2, 3, 4, 5], 1000),
                                          ((4, 4, 4, 4), [11, 12, 13], 96), ((8, 8), [2, 7], 700),
-                                         ((2, 2, 2, 2), [12, 13, 14], 333)])
+                                         ((2, 2, 2, 2), [12, 13, 14], 333),
+                                         # shapes without a resident kernel: the generic kernel's ensemble mode (Tab. I / III
+                                         # volumes 2^2, 6^2, 2^3, 8^3; an odd and a mixed lattice)
+                                         ((2, 2), [1, 2, 3], 300), ((6, 6), [1, 2, 3, 4], 500), ((2, 2, 2), [5, 6], 301),
+                                         ((8, 8, 8), [3, 4], 40), ((3, 3), [1, 2], 200), ((3, 2), [7, 8, 9], 100)])
 def test_ensemble_one_launch_matches_single_orbits_and_oracle(b, oracle, ext, seeds, n):
     """n_orbits orbits of one shape in ONE u1gf_relax_ensemble call == one u1gf_relax_batch call per orbit == the oracle,
     start by start (n is not a multiple of 32: the padding of each orbit's last batch must not leak); per-orbit copy
@@ -41,6 +45,7 @@ def test_ensemble_one_launch_matches_single_orbits_and_oracle(b, oracle, ext, se
     assert ens.n_orbits == len(seeds)
     r = b.relax_ensemble(ens, n)
     assert b.last_launch_count() == 1                      # one kernel for the whole ensemble
+    assert ens.orbit(0).kernel_name.startswith("lanes_") or ens.orbit(0).kernel_name.startswith("generic"), ens.orbit(0).kernel_name
     c = b.count_copies_ensemble(r["F_norm"], r["sig"], r["status"], nbins=100)
     for k, (th, seed) in enumerate(zip(thetas, seeds)):
         single = b.relax_batch(b.Orbit(ext, th), seed, n)
@@ -67,8 +72,6 @@ def test_ensemble_one_launch_matches_single_orbits_and_oracle(b, oracle, ext, se
         if nd <= 40:
             assert int(f["n_in_region"].item()) == sum(1 for _, ro in regions if ro != 0)
     ens.close()
-    with pytest.raises(b.U1gfError):
-        b.Ensemble((6, 6), np.zeros((2, 72)), [1, 2])       # no resident kernel for this shape
     torch.cuda.synchronize()
 
 
