@@ -264,7 +264,12 @@ int u1gf_release_host_scratch(void);
  *                          relaxed with the skip rule (the generic kernel applies the skip rule as always).
  *   u1gf_count_copies_ensemble   u1gf_count_copies per orbit on those arrays: copy ids, rep (positions) and
  *                          multiplicity are local to the orbit and stored at o * n_per_orbit; n_distinct dev
- *                          [n_orbits]; hist dev [n_orbits * nbins] or NULL; workspace >= u1gf_count_workspace_bytes(n_per_orbit)
+ *                          [n_orbits]; hist dev [n_orbits * nbins] or NULL; workspace >= u1gf_count_workspace_bytes(n_per_orbit):
+ *                          one u1gf_count_copies after the other on the orbits' slices.  With a workspace of at least
+ *                          u1gf_count_ensemble_onepass_workspace_bytes(n_orbits, n_per_orbit) bytes (0 = not available:
+ *                          one orbit, or n_orbits * n_per_orbit >= 2^31) all orbits are de-duplicated in ONE pass instead --
+ *                          records sorted by F, then stably by orbit index, runs cut at orbit boundaries -- with the same
+ *                          outputs bit for bit and a fixed number of launches whatever n_orbits is
  * ------------------------------------------------------------------------------------------------------- */
 typedef struct u1gf_ensemble u1gf_ensemble; /* opaque, library-owned */
 int u1gf_create_ensemble(int d, const int32_t* extents, int32_t n_orbits, const double* theta_host,
@@ -277,6 +282,7 @@ int u1gf_relax_ensemble(const u1gf_ensemble* e, uint64_t first_start, uint64_t n
                         double eps, int32_t max_sweeps, int32_t check_every, double* F_norm, int32_t* sweeps,
                         uint8_t* status, double* sig, void* workspace, size_t workspace_bytes, void* cuda_stream);
 size_t u1gf_count_ensemble_workspace_bytes(uint64_t n_per_orbit);
+size_t u1gf_count_ensemble_onepass_workspace_bytes(int32_t n_orbits, uint64_t n_per_orbit);
 int u1gf_count_copies_ensemble(int32_t n_orbits, uint64_t n_per_orbit, const double* F_norm, const double* sig,
                                const uint8_t* status, double tol_F, double tol_sig, int32_t* copy_id,
                                int64_t* n_distinct, int64_t* rep, int64_t* multiplicity, int64_t* hist, int32_t nbins,

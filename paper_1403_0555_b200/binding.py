@@ -52,6 +52,7 @@ _SIGNATURES = {
     "u1gf_relax_ensemble": (C.c_int, [_p, C.c_uint64, C.c_uint64, C.c_double, C.c_double, C.c_int32, C.c_int32, _p, _p, _p,
                                       _p, _p, C.c_size_t, _p]),
     "u1gf_count_ensemble_workspace_bytes": (C.c_size_t, [C.c_uint64]),
+    "u1gf_count_ensemble_onepass_workspace_bytes": (C.c_size_t, [C.c_int32, C.c_uint64]),
     "u1gf_count_copies_ensemble": (C.c_int, [C.c_int32, C.c_uint64, _p, _p, _p, C.c_double, C.c_double, _p, _p, _p, _p, _p,
                                              C.c_int32, _p, C.c_size_t, _p]),
     "u1gf_ensemble_stats": (C.c_int, [C.c_int32, C.c_uint64, _p, _p, _p, _p, _p, _p, _p]),
@@ -240,8 +241,9 @@ def relax_ensemble(ens: Ensemble, n_starts_per_orbit, *, first_start=0, omega=1.
     return out
 
 
-def count_copies_ensemble(F_norm, sig, status, tol_F=1e-10, tol_sig=1e-4, nbins=0, workspace=None):
-    """u1gf_count_copies_ensemble on [n_orbits, n] device tensors -> per-orbit tables ([n_orbits, n], n_distinct [n_orbits])."""
+def count_copies_ensemble(F_norm, sig, status, tol_F=1e-10, tol_sig=1e-4, nbins=0, workspace=None, one_pass=True):
+    """u1gf_count_copies_ensemble on [n_orbits, n] device tensors -> per-orbit tables ([n_orbits, n], n_distinct [n_orbits]).
+    one_pass: give the call the larger workspace with which it de-duplicates all orbits in one pass (where available)."""
     import torch
     no, n = int(F_norm.shape[0]), int(F_norm.shape[1])
     copy_id = torch.empty((no, n), dtype=torch.int32, device="cuda")
@@ -250,6 +252,8 @@ def count_copies_ensemble(F_norm, sig, status, tol_F=1e-10, tol_sig=1e-4, nbins=
     mult = torch.empty((no, max(n, 1)), dtype=torch.int64, device="cuda")
     hist = torch.empty((no, nbins), dtype=torch.int64, device="cuda") if nbins else None
     need = lib().u1gf_count_ensemble_workspace_bytes(n)
+    if one_pass:
+        need = max(need, lib().u1gf_count_ensemble_onepass_workspace_bytes(no, n))
     if workspace is None or workspace.numel() < need + 256:
         workspace = _workspace(need)
     _check(lib().u1gf_count_copies_ensemble(no, n, _dev_ptr(F_norm), _dev_ptr(sig), _dev_ptr(status), float(tol_F),

@@ -39,6 +39,9 @@ size_t cub_temp_bytes(size_t n) {
     cub::DeviceRadixSort::SortPairs(nullptr, a, (unsigned long long*)nullptr, (unsigned long long*)nullptr,
                                     (unsigned*)nullptr, (unsigned*)nullptr, (int)n);
     cub::DeviceScan::InclusiveSum(nullptr, b, (unsigned*)nullptr, (unsigned*)nullptr, (int)n);
+    size_t c = 0;   // the ensemble path's second, stable pass over 32-bit orbit indices
+    cub::DeviceRadixSort::SortPairs(nullptr, c, (unsigned*)nullptr, (unsigned*)nullptr, (unsigned*)nullptr, (unsigned*)nullptr, (int)n);
+    a = a > c ? a : c;
     return a > b ? a : b;
 }
 
@@ -180,6 +183,69 @@ __global__ void hist_kernel(const double* __restrict__ F, const int64_t* n_disti
     }
 }
 
+// ---- one pass over a whole ensemble: positions p = orbit * n_per + local position; the records are sorted by F and then,
+// stably, by orbit index, so that every orbit's converged records lie together in F order and the records that did not
+// converge (orbit key n_orbits) come last; a run never crosses an orbit boundary; leaders, and with them the global copy
+// ids, come out orbit by orbit, and the id inside the orbit is the global id minus the number of leaders before the orbit.
+__global__ void orbit_keys_kernel(unsigned n, unsigned n_per, unsigned n_orbits, const unsigned long long* __restrict__ keys_sorted,
+                                  const unsigned* __restrict__ pos_sorted, unsigned* __restrict__ okeys) {
+    const unsigned stride = gridDim.x * blockDim.x;
+    for (unsigned j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride)
+        okeys[j] = keys_sorted[j] == ~0ull ? n_orbits : pos_sorted[j] / n_per;
+}
+
+__global__ void run_flags_ens_kernel(unsigned n, unsigned n_per, const double* __restrict__ F, double tol_F, Work w) {
+    const unsigned n_conv = w.small[0];
+    const unsigned stride = gridDim.x * blockDim.x;
+    for (unsigned j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += stride) {
+        unsigned f = 0;
+        if (j < n_conv) {
+            const unsigned p = w.pos_out[j], q = j ? w.pos_out[j - 1] : 0u;
+            f = (j == 0 || p / n_per != q / n_per) ? 1u : ((F[p] - F[q] > tol_F) ? 1u : 0u);
+        }
+        w.run_id[j] = f;
+    }
+}
+
+__global__ void assign_ens_kernel(unsigned n, unsigned n_per, Work w, int32_t* copy_id, int64_t* n_distinct, int64_t* rep,
+                                  int64_t* multiplicity) {
+    const unsigned stride = gridDim.x * blockDim.x;
+    const unsigned nb = (n + 31) / 32 * 32;
+    for (unsigned p = blockIdx.x * blockDim.x + threadIdx.x; p < nb; p += stride) {
+        int gid = -1;
+        unsigned long long slot = 0;
+        if (p < n) {
+            const unsigned o = p / n_per, first = o * n_per;
+            const unsigned base = w.lead_idx[first];   // leaders before this orbit (exclusive scan at its first position)
+            const int lead = w.leader_of[p];
+            int id = -1;
+            if (lead >= 0) {
+                gid = (int)w.lead_idx[lead];
+                id = gid - (int)base;
+                slot = (unsigned long long)first + (unsigned)id;
+            }
+            copy_id[p] = id;
+            if (lead == (int)p) rep[slot] = (int64_t)(p - first);
+            if (p == first + n_per - 1) n_distinct[o] = (int64_t)w.lead_idx[p] + (lead == (int)p ? 1 : 0) - (int64_t)base;
+        }
+        const unsigned peers = __match_any_sync(0xffffffffu, gid);
+        if (gid >= 0 && (threadIdx.x & 31) == (unsigned)(__ffs(peers) - 1))
+            atomicAdd((unsigned long long*)&multiplicity[slot], (unsigned long long)__popc(peers));
+    }
+}
+
+__global__ void hist_ens_kernel(unsigned n, unsigned n_per, const double* __restrict__ F, const int64_t* __restrict__ n_distinct,
+                                const int64_t* __restrict__ rep, const int64_t* __restrict__ multiplicity, int64_t* hist, int nbins) {
+    const unsigned stride = gridDim.x * blockDim.x;
+    for (unsigned p = blockIdx.x * blockDim.x + threadIdx.x; p < n; p += stride) {
+        const unsigned o = p / n_per, c = p - o * n_per;
+        if ((int64_t)c >= n_distinct[o]) continue;
+        long long b = (long long)floor(F[(size_t)o * n_per + (size_t)rep[p]] * (double)nbins);
+        b = b < 0 ? 0 : (b > nbins - 1 ? nbins - 1 : b);
+        atomicAdd((unsigned long long*)&hist[(size_t)o * nbins + b], (unsigned long long)multiplicity[p]);
+    }
+}
+
 __global__ void init_small_kernel(unsigned* small, unsigned n) {
     if (threadIdx.x == 0) {
         small[0] = 0u;
@@ -196,6 +262,73 @@ __global__ void empty_kernel(int64_t* n_distinct, int64_t* hist, int nbins) {
 }
 
 }  // namespace
+
+size_t count_ens_onepass_workspace_bytes(unsigned n_orbits, uint64_t n_per) {
+    const unsigned long long n = (unsigned long long)n_orbits * n_per;
+    if (n == 0 || n >= (1ull << 31)) return 0;
+    Work w;
+    return carve(w, (size_t)n, nullptr);
+}
+
+// u1gf_count_copies for all orbits of an ensemble at once (same outputs as the per-orbit loop of ensemble.cu).
+int count_copies_ens_onepass(unsigned n_orbits, unsigned n_per, const double* F_norm, const double* sig, const uint8_t* status,
+                             double tol_F, double tol_sig, int32_t* copy_id, int64_t* n_distinct, int64_t* rep,
+                             int64_t* multiplicity, int64_t* hist, int nbins, void* workspace, cudaStream_t st) {
+    const unsigned n = n_orbits * n_per;
+    Work w;
+    carve(w, n, (char*)workspace);
+    int dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const unsigned blocks = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)sms * 8);
+    int launches = 0;
+    init_small_kernel<<<1, 32, 0, st>>>(w.small, n);
+    U1GF_CUDA(cudaGetLastError());
+    make_keys_kernel<<<blocks, 256, 0, st>>>(n, F_norm, status, w, multiplicity, hist, hist ? (int)n_orbits * nbins : 0);
+    U1GF_CUDA(cudaGetLastError());
+    launches += 2;
+    size_t tb = w.cub_bytes;
+    U1GF_CUDA(cub::DeviceRadixSort::SortPairs(w.cub_tmp, tb, w.keys_in, w.keys_out, w.pos_in, w.pos_out, (int)n, 0, 64, st));
+    // second, stable pass: orbit index as the major key.  The 64-bit input keys are no longer needed: their array holds
+    // the two 32-bit key arrays of this pass; the positions go back into pos_in, which becomes the sorted order
+    unsigned* ok_in = (unsigned*)w.keys_in;
+    unsigned* ok_out = ok_in + n;
+    orbit_keys_kernel<<<blocks, 256, 0, st>>>(n, n_per, n_orbits, w.keys_out, w.pos_out, ok_in);
+    U1GF_CUDA(cudaGetLastError());
+    ++launches;
+    int bits = 1;
+    while ((1u << bits) <= n_orbits) ++bits;
+    tb = w.cub_bytes;
+    U1GF_CUDA(cub::DeviceRadixSort::SortPairs(w.cub_tmp, tb, ok_in, ok_out, w.pos_out, w.pos_in, (int)n, 0, bits, st));
+    std::swap(w.pos_in, w.pos_out);
+    run_flags_ens_kernel<<<blocks, 256, 0, st>>>(n, n_per, F_norm, tol_F, w);
+    U1GF_CUDA(cudaGetLastError());
+    ++launches;
+    tb = w.cub_bytes;
+    U1GF_CUDA(cub::DeviceScan::InclusiveSum(w.cub_tmp, tb, w.run_id, w.run_id, (int)n, st));
+    {
+        int per_sm = 0;
+        U1GF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, elect_kernel, 256, 0));
+        unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)per_sm * sms);
+        if (grid < 1) grid = 1;
+        void* args[] = {(void*)&sig, (void*)&tol_sig, (void*)&w};
+        U1GF_CUDA(cudaLaunchCooperativeKernel((void*)elect_kernel, dim3(grid), dim3(256), args, 0, st));
+        ++launches;
+    }
+    tb = w.cub_bytes;
+    U1GF_CUDA(cub::DeviceScan::ExclusiveSum(w.cub_tmp, tb, w.lead_idx, w.lead_idx, (int)n, st));
+    assign_ens_kernel<<<blocks, 256, 0, st>>>(n, n_per, w, copy_id, n_distinct, rep, multiplicity);
+    U1GF_CUDA(cudaGetLastError());
+    ++launches;
+    if (hist) {
+        hist_ens_kernel<<<blocks, 256, 0, st>>>(n, n_per, F_norm, n_distinct, rep, multiplicity, hist, nbins);
+        U1GF_CUDA(cudaGetLastError());
+        ++launches;
+    }
+    t_launches = launches;
+    return U1GF_OK;
+}
+
 }  // namespace u1gf
 
 using namespace u1gf;

@@ -3,7 +3,8 @@
 // L213-220), one lattice per thread block with the grid over samples (L121).  Here the resident lane-per-start kernels
 // (relax_lanes.cu) number their 32-start batches over all orbits of the ensemble; a team of 32 lanes works through its
 // batches orbit by orbit and reloads the link table in shared memory at an orbit boundary.  De-duplication is per
-// orbit (copies of different orbits are unrelated), as a loop over u1gf_count_copies on the orbits' slices.
+// orbit (copies of different orbits are unrelated): in one pass with the orbit index as the major sort key when the caller's
+// workspace is large enough for all records (count_copies.cu), else as a loop over u1gf_count_copies on the orbits' slices.
 // Shapes without a resident kernel (2x2, 6x6, 2^3, 8^3, odd extents, ...) run on the generic kernel, one CTA per start
 // with the grid over the starts of all orbits -- the paper's own mapping.
 #include <new>
@@ -117,12 +118,30 @@ int u1gf_relax_ensemble(const u1gf_ensemble* e, uint64_t first_start, uint64_t n
 }
 
 size_t u1gf_count_ensemble_workspace_bytes(uint64_t n_per_orbit) { return u1gf_count_workspace_bytes(n_per_orbit); }
+size_t u1gf_count_ensemble_onepass_workspace_bytes(int32_t n_orbits, uint64_t n_per_orbit) {
+    return n_orbits > 1 ? count_ens_onepass_workspace_bytes((unsigned)n_orbits, n_per_orbit) : 0;
+}
 
 int u1gf_count_copies_ensemble(int32_t n_orbits, uint64_t n_per_orbit, const double* F_norm, const double* sig,
                                const uint8_t* status, double tol_F, double tol_sig, int32_t* copy_id,
                                int64_t* n_distinct, int64_t* rep, int64_t* multiplicity, int64_t* hist, int32_t nbins,
                                void* workspace, size_t workspace_bytes, void* cuda_stream) {
     if (n_orbits < 0) return fail(U1GF_EINVAL, "u1gf_count_copies_ensemble: n_orbits < 0");
+    // one pass over all orbits when the workspace is large enough for it (u1gf_count_ensemble_onepass_workspace_bytes)
+    const size_t onepass = n_orbits > 1 ? count_ens_onepass_workspace_bytes((unsigned)n_orbits, n_per_orbit) : 0;
+    if (onepass && workspace && workspace_bytes >= onepass) {
+        t_launches = 0;
+        if (!n_distinct || !F_norm || !sig || !status || !copy_id || !rep || !multiplicity)
+            return fail(U1GF_EINVAL, "u1gf_count_copies_ensemble: NULL array");
+        if (hist && nbins < 1) return fail(U1GF_EINVAL, "u1gf_count_copies_ensemble: nbins must be >= 1 when hist is given");
+        if (hist && (unsigned long long)n_orbits * (unsigned long long)nbins >= (1ull << 31))
+            return fail(U1GF_EINVAL, "u1gf_count_copies_ensemble: n_orbits * nbins must be below 2^31");
+        if (!(tol_F >= 0.0) || !(tol_sig >= 0.0)) return fail(U1GF_EINVAL, "u1gf_count_copies_ensemble: negative tolerance");
+        if (((uintptr_t)workspace & 255) != 0) return fail(U1GF_EINVAL, "u1gf_count_copies_ensemble: workspace not 256-byte aligned");
+        if (int rc = check_device()) return rc;
+        return count_copies_ens_onepass((unsigned)n_orbits, (unsigned)n_per_orbit, F_norm, sig, status, tol_F, tol_sig, copy_id,
+                                        n_distinct, rep, multiplicity, hist, nbins, workspace, (cudaStream_t)cuda_stream);
+    }
     int launches = 0;
     const size_t n = (size_t)n_per_orbit;
     for (int32_t k = 0; k < n_orbits; ++k) {   // the same workspace serves the orbits one after the other (stream order)

@@ -135,6 +135,11 @@ struct RelaxArgs {
 
 size_t generic_workspace_bytes(const u1gf_orbit* o, uint64_t n);
 int generic_relax(const u1gf_orbit* o, const RelaxArgs& a, cudaStream_t st);
+// count_copies.cu: the de-duplication of all orbits of an ensemble in one pass (ensemble.cu picks it when the workspace allows)
+size_t count_ens_onepass_workspace_bytes(unsigned n_orbits, uint64_t n_per);
+int count_copies_ens_onepass(unsigned n_orbits, unsigned n_per, const double* F_norm, const double* sig, const uint8_t* status,
+                             double tol_F, double tol_sig, int32_t* copy_id, int64_t* n_distinct, int64_t* rep,
+                             int64_t* multiplicity, int64_t* hist, int nbins, void* workspace, cudaStream_t st);
 // ensemble mode of the same kernel: n_orbits orbits of o's shape, links [n_orbits][V*d] at U_all, a.n_starts starts each
 int generic_relax_ens(const u1gf_orbit* o, const double2* U_all, const unsigned long long* seeds, unsigned n_orbits,
                       const RelaxArgs& a, cudaStream_t st);

@@ -46,7 +46,22 @@ def test_ensemble_one_launch_matches_single_orbits_and_oracle(b, oracle, ext, se
     r = b.relax_ensemble(ens, n)
     assert b.last_launch_count() == 1                      # one kernel for the whole ensemble
     assert ens.orbit(0).kernel_name.startswith("lanes_") or ens.orbit(0).kernel_name.startswith("generic"), ens.orbit(0).kernel_name
-    c = b.count_copies_ensemble(r["F_norm"], r["sig"], r["status"], nbins=100)
+    c = b.count_copies_ensemble(r["F_norm"], r["sig"], r["status"], nbins=100)            # all orbits in one pass
+    launches_one_pass = b.last_launch_count()
+    st_mixed = r["status"].clone()
+    st_mixed[:, 5::7] |= 1                                                                  # some records not converged
+    st_mixed[-1, :] |= 1                                                                    # the last orbit: none converged
+    for st_ in (r["status"], st_mixed):
+        c1 = b.count_copies_ensemble(r["F_norm"], r["sig"], st_, nbins=100)
+        cl = b.count_copies_ensemble(r["F_norm"], r["sig"], st_, nbins=100, one_pass=False)    # one u1gf_count_copies per orbit
+        nd1 = _cpu(c1["n_distinct"])
+        assert (nd1 == _cpu(cl["n_distinct"])).all() and (_cpu(c1["copy_id"]) == _cpu(cl["copy_id"])).all()
+        assert (_cpu(c1["hist"]) == _cpu(cl["hist"])).all()
+        for k in range(len(seeds)):
+            for key in ("rep", "multiplicity"):
+                assert (_cpu(c1[key][k])[:nd1[k]] == _cpu(cl[key][k])[:nd1[k]]).all(), (k, key)
+    assert nd1[-1] == 0 and (_cpu(c1["copy_id"][-1]) == -1).all()
+    assert b.last_launch_count() > launches_one_pass or len(seeds) == 1                    # the loop launches per orbit
     for k, (th, seed) in enumerate(zip(thetas, seeds)):
         single = b.relax_batch(b.Orbit(ext, th), seed, n)
         o = oracle.relax(ext, th, seed, n)
