@@ -479,7 +479,40 @@ def main():
             t_ms, r_ms, f_ms = time_pipeline(p2, torch, flush, csteps, cwarm + (1 if cid == 5 and oi >= 2 else 0))
             s2, _, _, _ = p2.summary(r_ms, f_ms, float(np.median(time_pipeline.last_per_step)), peak_dfma, sm_clock, sms, hbm_peak)
             s2.update(steps=csteps, warmup=cwarm, ms_per_step_is="median of the timed steps")
+            if cid == 5 and oi == 2:
+                # the one-call host API on a hot orbit (most starts are their own copy): the handle's second and later calls
+                # keep the fields of all starts from the first pass instead of relaxing the representatives again
+                n2, V2 = o2["n_starts"], synth.volume(o2["extents"])
+                hb2 = b.host_buffers(n2)
+                orb2 = b.Orbit(o2["extents"], p2.theta)
+                kw2 = dict(p2.kw, nbins=10000, out=hb2)
+                b.pipeline_host(orb2, o2["seed"], n2, **kw2)      # first call on the handle: learns that the orbit is hot
+                b.pipeline_host(orb2, o2["seed"], n2, **kw2)
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                for _ in range(csteps):
+                    ph = b.pipeline_host(orb2, o2["seed"], n2, **kw2)
+                dt = (time.perf_counter() - t0) / csteps
+                su2 = float(V2) * float(ph["sweeps"].sum(dtype=np.int64))
+                nd2 = ph["n_distinct"]
+                s2["e2e"] = {"value": su2 / dt, "unit": UNIT, "ms_per_call": dt * 1e3, "fraction_of_value": su2 / dt / s2["value"],
+                             "h2d_bytes_per_step": 0, "d2h_bytes_per_step": int(n2 * (8 + 4 + 1 + 32 + 4) + 16 + nd2 * 33 + 80000),
+                             "call": "u1gf_pipeline_host on an existing handle (third and later calls), pinned per-start arrays",
+                             "gpu_launches": b.last_launch_count(), "n_distinct": nd2, "n_in_first_region": ph["n_in_region"]}
+                del hb2, orb2, ph
+                b.lib().u1gf_release_host_scratch()
             configs[f"cfg{cid}_{'x'.join(map(str, o2['extents']))}"] = s2
+            del p2
+            torch.cuda.empty_cache()
+        # the paper's other volumes (Tab. I, Tab. III): hot orbits, seed 21, not BASELINE configs
+        for ext2, n2 in (((10, 10), 1 << 20), ((6, 6, 6), 1 << 20), ((8, 8, 8), 1 << 18)):
+            c2 = dict(name="paper_volume", omega=1.7, eps=1e-13, max_sweeps=20000)
+            o2 = dict(extents=ext2, kind="uniform", seed=21, n_starts=n2)
+            p2 = Pipeline(b, torch, c2, o2, 0)
+            t_ms, r_ms, f_ms = time_pipeline(p2, torch, flush, csteps, cwarm + 1)
+            s2, _, _, _ = p2.summary(r_ms, f_ms, float(np.median(time_pipeline.last_per_step)), peak_dfma, sm_clock, sms, hbm_peak)
+            s2.update(steps=csteps, warmup=cwarm + 1, ms_per_step_is="median of the timed steps")
+            configs[f"paper_volume_{'x'.join(map(str, ext2))}"] = s2
             del p2
             torch.cuda.empty_cache()
         configs["cfg3_ensemble"] = ensemble_config3(b, torch, flush, csteps, cwarm, peak_dfma, sm_clock, sms)
